@@ -1,0 +1,167 @@
+"""CPU oracle -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Thin ctypes loader for ``oracle/gw_oracle.c`` (plain C, fp64, libm), the slow and
+obviously-correct statement of what the hot path computes (Eq. 1,
+PAPER.md:69 time shift; waveform per BASELINE.json north_star, written out in
+SURVEY.md 8(c) O1..O7).  Only ``tests/``, ``__graft_entry__.smoke()`` and the
+``cpu_baseline`` / ``--impl reference`` leg of ``bench.py`` may import this
+package.  It imports nothing from ``paper_1904_02863_b200`` and shares no code
+with the CUDA path.  All marshalling below is argument plumbing: every number is
+computed inside ``gw_oracle.c``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gw_oracle.c")
+_LIB = os.path.join(_HERE, "libgw_oracle.so")
+
+NPARAM = 11          # Mc, q, chi1, chi2, DL, tc, phic, cos(iota), ra, dec, psi
+DET_ROW = 13         # kind, vertex[3], xarm[3], yarm[3], fplus, fcross, dt
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile gw_oracle.c with gcc (-O2, no fast-math, OpenMP over proposals)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+               "-Wall", "-Wextra", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    build()
+    lib = ctypes.CDLL(_LIB)
+    dp = ctypes.POINTER(ctypes.c_double)
+    i64, cint, dbl = ctypes.c_int64, ctypes.c_int, ctypes.c_double
+    lib.gwo_constants.argtypes = [dp]
+    lib.gwo_masses.argtypes = [dbl, dbl, dp, dp, dp, dp]
+    lib.gwo_phase_coefficients.argtypes = [dbl, dbl, dbl, dbl, dbl, cint, dp, dp]
+    lib.gwo_phase.argtypes = [dbl, dp, cint]
+    lib.gwo_phase.restype = dbl
+    lib.gwo_amplitude.argtypes = [dbl, dbl]
+    lib.gwo_amplitude.restype = dbl
+    lib.gwo_antenna.argtypes = [dp, dbl, dbl, dbl, dbl, dp, dp, dp]
+    lib.gwo_sky_frame.argtypes = [dbl, dbl, dbl, dbl, dp, dp, dp]
+    lib.gwo_waveform.argtypes = [i64, dp, cint, dp, dbl, i64, dp, cint, dp]
+    lib.gwo_lnl.argtypes = [i64, dp, dbl, cint, dp, dp, dp, dbl, i64, dp, cint, cint, dp, dp]
+    lib.gwo_lnl.restype = cint
+    lib.gwo_inner.argtypes = [i64, dbl, dp, dp, dp, dp, dp]
+    lib.gwo_norm_i7.argtypes = [i64, dp, dbl, dp]
+    lib.gwo_norm_i7.restype = dbl
+    _lib = lib
+    return lib
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _f64(a, shape=None) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if shape is not None:
+        a = a.reshape(shape)
+    return a
+
+
+def _ri(z) -> np.ndarray:
+    """complex128 array -> contiguous float64 view with trailing (re, im)."""
+    z = np.ascontiguousarray(z, dtype=np.complex128)
+    return z.view(np.float64).reshape(z.shape + (2,))
+
+
+def constants() -> dict:
+    out = np.zeros(4)
+    _load().gwo_constants(_p(out))
+    return {"tsun_s": out[0], "mpc_s": out[1], "c_si": out[2], "euler_gamma": out[3]}
+
+
+def masses(mc: float, q: float):
+    """O1 -> (eta, M_s [s], mu1, mu2)."""
+    vals = [ctypes.c_double() for _ in range(4)]
+    _load().gwo_masses(mc, q, *[ctypes.byref(v) for v in vals])
+    return tuple(v.value for v in vals)
+
+
+def phase_coefficients(eta, mu1, mu2, chi1=0.0, chi2=0.0, spin_order=1):
+    """O2 -> (phi[8], phil[8])."""
+    phi, phil = np.zeros(8), np.zeros(8)
+    _load().gwo_phase_coefficients(eta, mu1, mu2, chi1, chi2, spin_order, _p(phi), _p(phil))
+    return phi, phil
+
+
+def phase(freqs, theta, spin_order=1) -> np.ndarray:
+    """O3: Psi(f) for one theta[11] at each frequency."""
+    lib = _load()
+    th = _f64(theta, (NPARAM,))
+    return np.array([lib.gwo_phase(float(f), _p(th), spin_order) for f in np.atleast_1d(freqs)])
+
+
+def amplitude(mc: float, dl: float) -> float:
+    """O4: A0."""
+    return _load().gwo_amplitude(mc, dl)
+
+
+def antenna(det_row, ra, dec, psi, gmst):
+    """O6 -> (F+, Fx, dt_s) for one detector row."""
+    d = _f64(det_row, (DET_ROW,))
+    vals = [ctypes.c_double() for _ in range(3)]
+    _load().gwo_antenna(_p(d), ra, dec, psi, gmst, *[ctypes.byref(v) for v in vals])
+    return tuple(v.value for v in vals)
+
+
+def sky_frame(ra, dec, psi, gmst):
+    """O6 -> (X, Y, n) unit vectors."""
+    X, Y, n = np.zeros(3), np.zeros(3), np.zeros(3)
+    _load().gwo_sky_frame(ra, dec, psi, gmst, _p(X), _p(Y), _p(n))
+    return X, Y, n
+
+
+def waveform(freqs, dets, gmst, theta, spin_order=1) -> np.ndarray:
+    """O4..O6: h[n_prop][n_det][n_bins] complex128."""
+    f = _f64(freqs)
+    d = _f64(dets).reshape(-1, DET_ROW)
+    th = _f64(theta).reshape(-1, NPARAM)
+    out = np.empty((th.shape[0], d.shape[0], f.shape[0], 2))
+    _load().gwo_waveform(f.shape[0], _p(f), d.shape[0], _p(d), gmst, th.shape[0], _p(th),
+                         spin_order, _p(out))
+    return out.view(np.complex128)[..., 0]
+
+
+def lnl(freqs, delta_f, data, psd, dets, gmst, theta, spin_order=1, n_threads=0):
+    """O7 -> (lnL[n_prop], parts[n_prop][n_det][3], threads_used)."""
+    f = _f64(freqs)
+    d = _f64(dets).reshape(-1, DET_ROW)
+    n_det, n_bins = d.shape[0], f.shape[0]
+    dat = _ri(np.asarray(data).reshape(n_det, n_bins))
+    S = _f64(psd, (n_det, n_bins))
+    th = _f64(theta).reshape(-1, NPARAM)
+    out = np.empty(th.shape[0])
+    parts = np.empty((th.shape[0], n_det, 3))
+    used = _load().gwo_lnl(n_bins, _p(f), float(delta_f), n_det, _p(dat), _p(S), _p(d), gmst,
+                           th.shape[0], _p(th), spin_order, int(n_threads), _p(out), _p(parts))
+    return out, parts, used
+
+
+def inner(delta_f, a, b, psd) -> complex:
+    """<a|b> = 4 df sum a conj(b)/S for one detector."""
+    a_, b_, S = _ri(np.ravel(a)), _ri(np.ravel(b)), _f64(np.ravel(psd))
+    re, im = ctypes.c_double(), ctypes.c_double()
+    _load().gwo_inner(S.shape[0], float(delta_f), _p(a_), _p(b_), _p(S), ctypes.byref(re), ctypes.byref(im))
+    return complex(re.value, im.value)
+
+
+def norm_i7(freqs, delta_f, psd) -> float:
+    """I7 = 4 df sum f^(-7/3)/S."""
+    f, S = _f64(freqs), _f64(psd)
+    return _load().gwo_norm_i7(f.shape[0], _p(f), float(delta_f), _p(S))
