@@ -1,0 +1,433 @@
+// gw_api.cu -- the C-ABI of include/gwlnl.h: context lifetime, input validation, launch planning and the
+// batch entry points.  Every step of the hot path runs in the kernels of gw_kernels.cu; this file only
+// validates, allocates (create/reserve only) and launches.  There is no CPU fallback.
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "gw_internal.h"
+
+using namespace gw;
+
+struct gw_ctx {
+    int          device;
+    int          n_sm;
+    int          ctas_per_sm;      // resident fused CTAs per SM for this n_det
+    int          spin_order;
+    double       gmst;
+    DetSet       dets;
+    Tables       t;
+    Workspace    w;
+    int          last_cuda_error;
+    int64_t      launches;
+};
+
+namespace {
+
+constexpr int64_t kHStageMaxDoubles = (int64_t)1 << 26;       // 512 MiB waveform slab for the host variant
+
+int cuda_fail(gw_ctx *ctx, cudaError_t e)
+{
+    if (ctx) ctx->last_cuda_error = (int)e;
+    return e == cudaErrorMemoryAllocation ? GW_ERR_ALLOC : GW_ERR_CUDA;
+}
+
+bool is_device_ptr(const void *p)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+// ---- launch planning -----------------------------------------------------------------------------------
+// Cost model: a CTA sweeps ceil(chunk/lpp) bins per thread plus a fixed prologue /
+// epilogue worth ~kProBins bins; an SM runs its resident CTAs concurrently and the fp64 pipe saturates at
+// about kSatWarps warps per scheduler.  The plan is a pure function of (n_prop, M, n_det, device), which is
+// what makes the summation order reproducible.
+constexpr double kProBins  = 14.0;
+constexpr double kSatWarps = 3.0;
+constexpr int    kMaxChunks = 4096;
+constexpr int64_t kMaxWaves = 8;
+
+Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
+{
+    const int64_t M = ctx->t.n_bins;
+    const int slots_per_sm = ctx->ctas_per_sm > 0 ? ctx->ctas_per_sm : 1;
+    const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 148;
+    const int64_t slots = (int64_t)n_sm * slots_per_sm;
+    Plan best = {1, kThreads, 1, (n_prop + kThreads - 1) / kThreads};
+    double best_cost = 1e300;
+    for (int lpp = 1; lpp <= 32; lpp *= 2) {
+        const int pt = kThreads / lpp;
+        const int64_t tiles = (n_prop + pt - 1) / pt;
+        int64_t max_chunks = M / ((int64_t)8 * lpp);          // at least 8 iterations per thread
+        const int64_t by_waves = (kMaxWaves * slots) / tiles; // no more than kMaxWaves waves of CTAs
+        if (max_chunks > by_waves) max_chunks = by_waves;
+        if (max_chunks > kMaxChunks) max_chunks = kMaxChunks;
+        if (max_chunks < 1) max_chunks = 1;
+        for (int64_t nc = 1; nc <= max_chunks; ++nc) {
+            const int64_t ctas = tiles * nc;
+            const int64_t chunk = (M + nc - 1) / nc;
+            const double per_thread = (double)((chunk + lpp - 1) / lpp) + kProBins + (lpp > 1 ? 2.0 : 0.0);
+            const int64_t per_sm = (ctas + n_sm - 1) / n_sm;                  // CTAs an SM must run
+            const int64_t waves = (per_sm + slots_per_sm - 1) / slots_per_sm;
+            const double resident = (double)per_sm / (double)waves;           // average co-resident CTAs
+            const double warps_per_sched = resident * (kThreads / 32) / 4.0;
+            const double slowdown = warps_per_sched > kSatWarps ? warps_per_sched / kSatWarps : 1.0;
+            const double cost = (double)waves * per_thread * slowdown + 1e-3 * (double)nc;
+            if (cost < best_cost) {
+                best_cost = cost;
+                best.lpp = lpp; best.props_per_cta = pt; best.n_chunks = (int)nc; best.n_tiles = tiles;
+            }
+        }
+        if (tiles >= slots) break;                            // enough proposals to fill the GPU: keep this lpp
+    }
+    return best;
+}
+
+// upper bound of partial_need over every plan make_plan can return for n_prop <= max_batch
+int64_t partial_bound(const gw_ctx *ctx, int64_t max_batch)
+{
+    const int slots_per_sm = ctx->ctas_per_sm > 0 ? ctx->ctas_per_sm : 1;
+    const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 148;
+    const int64_t ctas = kMaxWaves * (int64_t)n_sm * slots_per_sm + (max_batch + kThreads - 1) / kThreads + 1;
+    return ctas * kThreads * (int64_t)(2 * ctx->t.n_det);
+}
+
+int64_t partial_need(const gw_ctx *ctx, const Plan &p)
+{
+    return p.n_chunks > 1 ? p.n_tiles * p.n_chunks * (int64_t)(2 * ctx->t.n_det) * p.props_per_cta : 0;
+}
+
+void free_workspace(Workspace &w)
+{
+    cudaFree(w.rec); cudaFree(w.partial); cudaFree(w.tickets); cudaFree(w.theta_stage);
+    cudaFree(w.lnl_stage); cudaFree(w.parts_stage); cudaFree(w.h_stage);
+    std::memset(&w, 0, sizeof(w));
+}
+
+int reserve_impl(gw_ctx *ctx, int64_t max_batch)
+{
+    if (max_batch <= ctx->w.max_batch) return GW_OK;
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    const int64_t need_partial = partial_bound(ctx, max_batch);
+    const int64_t need_tickets = (max_batch + 7) / 8 + 1;     // tiles at lpp = 32
+    Workspace w;
+    std::memset(&w, 0, sizeof(w));
+    w.max_batch = max_batch;
+    w.rec_stride = (max_batch + 31) / 32 * 32;
+    const int n_det = ctx->t.n_det;
+    const int64_t n_rec = 9 + kRecPerDet * n_det;
+    w.partial_doubles = need_partial > 0 ? need_partial : 1;
+    w.n_tickets = need_tickets;
+    w.h_stage_doubles = 0;                                    // the host waveform variant allocates its slab on first use
+    bool ok = true;
+    ok = ok && (e = cudaMalloc(&w.rec, sizeof(double) * n_rec * w.rec_stride)) == cudaSuccess;
+    ok = ok && (e = cudaMalloc(&w.partial, sizeof(double) * w.partial_doubles)) == cudaSuccess;
+    ok = ok && (e = cudaMalloc(&w.tickets, sizeof(unsigned int) * w.n_tickets)) == cudaSuccess;
+    ok = ok && (e = cudaMalloc(&w.theta_stage, sizeof(double) * max_batch * GW_NPARAM)) == cudaSuccess;
+    ok = ok && (e = cudaMalloc(&w.lnl_stage, sizeof(double) * max_batch)) == cudaSuccess;
+    ok = ok && (e = cudaMalloc(&w.parts_stage, sizeof(double) * max_batch * n_det * 3)) == cudaSuccess;
+    ok = ok && (e = cudaMemset(w.tickets, 0, sizeof(unsigned int) * w.n_tickets)) == cudaSuccess;
+    if (!ok) {
+        free_workspace(w);
+        cudaGetLastError();
+        return cuda_fail(ctx, e);
+    }
+    double *old_h = ctx->w.h_stage;
+    const int64_t old_h_doubles = ctx->w.h_stage_doubles;
+    ctx->w.h_stage = nullptr;
+    free_workspace(ctx->w);
+    ctx->w = w;
+    ctx->w.h_stage = old_h;
+    ctx->w.h_stage_doubles = old_h_doubles;
+    return GW_OK;
+}
+
+bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
+
+int check_batch_args(gw_ctx *ctx, int64_t n_prop, const void *theta, const void *out)
+{
+    if (!ctx || n_prop < 0) return GW_ERR_INVALID_ARG;
+    if (n_prop == 0) return GW_OK;
+    if (!theta || !out) return GW_ERR_INVALID_ARG;
+    if (n_prop > ctx->w.max_batch) return GW_ERR_INVALID_ARG;
+    return GW_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int gw_abi_version(void) { return GW_ABI_VERSION; }
+
+const char *gw_strerror(int code)
+{
+    switch (code) {
+    case GW_OK:              return "ok";
+    case GW_ERR_INVALID_ARG: return "invalid argument";
+    case GW_ERR_ALLOC:       return "allocation failed";
+    case GW_ERR_CUDA:        return "CUDA runtime error";
+    case GW_ERR_ARCH:        return "device is not compute capability 10.x (sm_100a)";
+    default:                 return "unknown error code";
+    }
+}
+
+int gw_last_cuda_error(const gw_ctx *ctx) { return ctx ? ctx->last_cuda_error : 0; }
+
+int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_det, const double *data_ri,
+                  const double *psd, const gw_detector *dets, double gmst_rad, const gw_options *opt,
+                  void *cuda_stream)
+{
+    if (!out) return GW_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!freqs_hz || !data_ri || !psd || !dets) return GW_ERR_INVALID_ARG;
+    if (n_bins < 2 || n_bins > ((int64_t)1 << 30) || n_det < 1 || n_det > GW_MAX_DET) return GW_ERR_INVALID_ARG;
+    if (!std::isfinite(gmst_rad)) return GW_ERR_INVALID_ARG;
+    gw_options o = {1, 0, 4096};
+    if (opt) o = *opt;
+    if (o.spin_order < 0 || o.spin_order > 1 || o.isco_cut != 0 || o.max_batch < 1) return GW_ERR_INVALID_ARG;
+
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return GW_ERR_CUDA;
+    cudaDeviceProp prop;
+    if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) return GW_ERR_CUDA;
+    if (prop.major != 10) return GW_ERR_ARCH;
+
+    // ---- host copies for validation (inputs may live on either side) ----
+    const size_t nf = (size_t)n_bins, nd = (size_t)n_det * n_bins;
+    std::vector<double> hf, hd, hp;
+    try { hf.resize(nf); hd.resize(nd * 2); hp.resize(nd); } catch (const std::bad_alloc &) { return GW_ERR_ALLOC; }
+    const cudaMemcpyKind kf = is_device_ptr(freqs_hz) ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost;
+    const cudaMemcpyKind kd = is_device_ptr(data_ri) ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost;
+    const cudaMemcpyKind kp = is_device_ptr(psd) ? cudaMemcpyDeviceToHost : cudaMemcpyHostToHost;
+    if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return GW_ERR_CUDA;
+    if ((e = cudaMemcpy(hf.data(), freqs_hz, nf * sizeof(double), kf)) != cudaSuccess) return GW_ERR_CUDA;
+    if ((e = cudaMemcpy(hd.data(), data_ri, nd * 2 * sizeof(double), kd)) != cudaSuccess) return GW_ERR_CUDA;
+    if ((e = cudaMemcpy(hp.data(), psd, nd * sizeof(double), kp)) != cudaSuccess) return GW_ERR_CUDA;
+
+    const double f0 = hf[0];
+    const double df = (hf[nf - 1] - hf[0]) / (double)(n_bins - 1);
+    if (!finite_pos(f0) || !finite_pos(df)) return GW_ERR_INVALID_ARG;
+    {
+        // uniform to rounding: the time-shift recurrence assumes f_j = f_0 + j df
+        const double tol = 1e-9 * df + 8.0 * std::ldexp(std::fabs(hf[nf - 1]), -52);
+        for (size_t j = 0; j < nf; ++j) {
+            if (!std::isfinite(hf[j]) || std::fabs(hf[j] - (f0 + (double)j * df)) > tol) return GW_ERR_INVALID_ARG;
+        }
+    }
+    for (size_t k = 0; k < nd; ++k) if (!finite_pos(hp[k])) return GW_ERR_INVALID_ARG;
+    for (size_t k = 0; k < nd * 2; ++k) if (!std::isfinite(hd[k])) return GW_ERR_INVALID_ARG;
+
+    gw_ctx *ctx = new (std::nothrow) gw_ctx;
+    if (!ctx) return GW_ERR_ALLOC;
+    std::memset(ctx, 0, sizeof(*ctx));
+    ctx->device = dev;
+    ctx->n_sm = prop.multiProcessorCount;
+    ctx->spin_order = o.spin_order;
+    ctx->gmst = gmst_rad;
+    for (int i = 0; i < n_det; ++i) {
+        const gw_detector &d = dets[i];
+        DetGeom &g = ctx->dets.d[i];
+        g.kind = d.kind;
+        if (d.kind == GW_DET_GEOMETRIC) {
+            double nx = 0, ny = 0;
+            for (int a = 0; a < 3; ++a) { nx += d.xarm[a] * d.xarm[a]; ny += d.yarm[a] * d.yarm[a]; }
+            bool fin = true;
+            for (int a = 0; a < 3; ++a) fin = fin && std::isfinite(d.vertex_m[a]);
+            if (!fin || !(std::fabs(nx - 1.0) <= 2e-6) || !(std::fabs(ny - 1.0) <= 2e-6)) { delete ctx; return GW_ERR_INVALID_ARG; }
+            const double *x = d.xarm, *y = d.yarm;
+            g.D[0] = 0.5 * (x[0] * x[0] - y[0] * y[0]); g.D[1] = 0.5 * (x[0] * x[1] - y[0] * y[1]);
+            g.D[2] = 0.5 * (x[0] * x[2] - y[0] * y[2]); g.D[3] = 0.5 * (x[1] * x[1] - y[1] * y[1]);
+            g.D[4] = 0.5 * (x[1] * x[2] - y[1] * y[2]); g.D[5] = 0.5 * (x[2] * x[2] - y[2] * y[2]);
+            for (int a = 0; a < 3; ++a) g.rc[a] = d.vertex_m[a] / 299792458.0;
+        } else if (d.kind == GW_DET_FIXED) {
+            if (!std::isfinite(d.fplus) || !std::isfinite(d.fcross) || !std::isfinite(d.dt_s)) { delete ctx; return GW_ERR_INVALID_ARG; }
+            g.fplus = d.fplus; g.fcross = d.fcross; g.dt_s = d.dt_s;
+        } else { delete ctx; return GW_ERR_INVALID_ARG; }
+    }
+
+    int rc = GW_OK;
+    double *dfreq = nullptr, *ddata = nullptr, *dpsd = nullptr, *di7 = nullptr;
+    Tables &t = ctx->t;
+    t.n_bins = n_bins; t.n_pad = (n_bins + 31) / 32 * 32 + 32; t.n_det = n_det; t.f0 = f0; t.delta_f = df;
+    do {
+        if ((e = configure_kernels(nullptr)) != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
+        ctx->ctas_per_sm = fused_ctas_per_sm(n_det);
+        bool ok = true;
+        ok = ok && (e = cudaMalloc(&t.planes, sizeof(double) * 2 * (kBasisPlanes + n_det) * t.n_pad)) == cudaSuccess;
+        ok = ok && (e = cudaMalloc(&t.fm76, sizeof(double) * t.n_pad)) == cudaSuccess;
+        ok = ok && (e = cudaMalloc(&t.freq, sizeof(double) * t.n_pad)) == cudaSuccess;
+        ok = ok && (e = cudaMalloc(&dfreq, sizeof(double) * nf)) == cudaSuccess;
+        ok = ok && (e = cudaMalloc(&ddata, sizeof(double) * nd * 2)) == cudaSuccess;
+        ok = ok && (e = cudaMalloc(&dpsd, sizeof(double) * nd)) == cudaSuccess;
+        ok = ok && (e = cudaMalloc(&di7, sizeof(double) * GW_MAX_DET)) == cudaSuccess;
+        if (!ok) { rc = cuda_fail(ctx, e); break; }
+        ok = ok && (e = cudaMemcpyAsync(dfreq, hf.data(), nf * sizeof(double), cudaMemcpyHostToDevice, s)) == cudaSuccess;
+        ok = ok && (e = cudaMemcpyAsync(ddata, hd.data(), nd * 2 * sizeof(double), cudaMemcpyHostToDevice, s)) == cudaSuccess;
+        ok = ok && (e = cudaMemcpyAsync(dpsd, hp.data(), nd * sizeof(double), cudaMemcpyHostToDevice, s)) == cudaSuccess;
+        if (!ok) { rc = cuda_fail(ctx, e); break; }
+        if ((e = launch_precompute(t, dfreq, ddata, dpsd, di7, s, &ctx->launches)) != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
+        if ((e = cudaMemcpyAsync(t.i7, di7, sizeof(double) * n_det, cudaMemcpyDeviceToHost, s)) != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
+        rc = reserve_impl(ctx, o.max_batch);
+    } while (0);
+    cudaFree(dfreq); cudaFree(ddata); cudaFree(dpsd); cudaFree(di7);
+    if (rc != GW_OK) {
+        gw_ctx_destroy(ctx);
+        cudaGetLastError();
+        return rc;
+    }
+    *out = ctx;
+    return GW_OK;
+}
+
+int gw_ctx_reserve(gw_ctx *ctx, int64_t max_batch)
+{
+    if (!ctx || max_batch < 1) return GW_ERR_INVALID_ARG;
+    return reserve_impl(ctx, max_batch);
+}
+
+int gw_ctx_destroy(gw_ctx *ctx)
+{
+    if (!ctx) return GW_OK;
+    cudaDeviceSynchronize();
+    free_workspace(ctx->w);
+    cudaFree(ctx->t.planes); cudaFree(ctx->t.fm76); cudaFree(ctx->t.freq);
+    delete ctx;
+    cudaGetLastError();
+    return GW_OK;
+}
+
+int gw_ctx_info(const gw_ctx *ctx, int64_t *n_bins, int *n_det, double *delta_f, int64_t *max_batch)
+{
+    if (!ctx) return GW_ERR_INVALID_ARG;
+    if (n_bins) *n_bins = ctx->t.n_bins;
+    if (n_det) *n_det = ctx->t.n_det;
+    if (delta_f) *delta_f = ctx->t.delta_f;
+    if (max_batch) *max_batch = ctx->w.max_batch;
+    return GW_OK;
+}
+
+int gw_ctx_plan(const gw_ctx *ctx, int64_t n_prop, int *lanes_per_prop, int *props_per_cta, int *n_chunks,
+                int64_t *n_ctas)
+{
+    if (!ctx || n_prop < 1) return GW_ERR_INVALID_ARG;
+    const Plan p = make_plan(ctx, n_prop);
+    if (lanes_per_prop) *lanes_per_prop = p.lpp;
+    if (props_per_cta) *props_per_cta = p.props_per_cta;
+    if (n_chunks) *n_chunks = p.n_chunks;
+    if (n_ctas) *n_ctas = p.n_tiles * p.n_chunks;
+    return GW_OK;
+}
+
+int gw_ctx_norms(const gw_ctx *ctx, double *i7_host)
+{
+    if (!ctx || !i7_host) return GW_ERR_INVALID_ARG;
+    for (int i = 0; i < ctx->t.n_det; ++i) i7_host[i] = ctx->t.i7[i];
+    return GW_OK;
+}
+
+int64_t gw_ctx_launch_count(const gw_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *lnl_out_dev,
+                 double *parts_out_dev, void *cuda_stream)
+{
+    int rc = check_batch_args(ctx, n_prop, theta_dev, lnl_out_dev);
+    if (rc != GW_OK || n_prop == 0) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const Plan p = make_plan(ctx, n_prop);
+    if (partial_need(ctx, p) > ctx->w.partial_doubles || p.n_tiles > ctx->w.n_tickets) return GW_ERR_INVALID_ARG;
+    cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
+                                 ctx->w.rec_stride, (double)p.lpp * ctx->t.delta_f, s, &ctx->launches);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    e = launch_fused(ctx->t, p, n_prop, ctx->w.rec, ctx->w.rec_stride, ctx->w.partial, ctx->w.tickets, lnl_out_dev,
+                     parts_out_dev, s, &ctx->launches);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return GW_OK;
+}
+
+int gw_waveform_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *h_out_dev, void *cuda_stream)
+{
+    int rc = check_batch_args(ctx, n_prop, theta_dev, h_out_dev);
+    if (rc != GW_OK || n_prop == 0) return rc;
+    if (((uintptr_t)h_out_dev & 15u) != 0) return GW_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
+                                 ctx->w.rec_stride, ctx->t.delta_f, s, &ctx->launches);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    e = launch_waveform(ctx->t, n_prop, ctx->w.rec, ctx->w.rec_stride, h_out_dev, s, &ctx->launches);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return GW_OK;
+}
+
+int gw_lnl_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, double *lnl_out_host,
+                      double *parts_out_host, void *cuda_stream)
+{
+    int rc = check_batch_args(ctx, n_prop, theta_host, lnl_out_host);
+    if (rc != GW_OK || n_prop == 0) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    Workspace &w = ctx->w;
+    cudaError_t e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * GW_NPARAM,
+                                    cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    rc = gw_lnl_batch(ctx, n_prop, w.theta_stage, w.lnl_stage, parts_out_host ? w.parts_stage : nullptr, cuda_stream);
+    if (rc != GW_OK) return rc;
+    e = cudaMemcpyAsync(lnl_out_host, w.lnl_stage, sizeof(double) * n_prop, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess && parts_out_host)
+        e = cudaMemcpyAsync(parts_out_host, w.parts_stage, sizeof(double) * n_prop * ctx->t.n_det * 3,
+                            cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    return GW_OK;
+}
+
+int gw_waveform_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, double *h_out_host,
+                           void *cuda_stream)
+{
+    int rc = check_batch_args(ctx, n_prop, theta_host, h_out_host);
+    if (rc != GW_OK || n_prop == 0) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    Workspace &w = ctx->w;
+    const int64_t per_prop = (int64_t)ctx->t.n_det * ctx->t.n_bins * 2;
+    cudaError_t e;
+    if (w.h_stage_doubles < per_prop) {                       // first use: allocate the slab (host variant only)
+        int64_t want = per_prop * n_prop;
+        if (want > kHStageMaxDoubles) want = (kHStageMaxDoubles / per_prop) * per_prop;
+        if (want < per_prop) want = per_prop;
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(ctx, e);
+        cudaFree(w.h_stage); w.h_stage = nullptr; w.h_stage_doubles = 0;
+        if ((e = cudaMalloc(&w.h_stage, sizeof(double) * want)) != cudaSuccess) { cudaGetLastError(); return cuda_fail(ctx, e); }
+        w.h_stage_doubles = want;
+    }
+    const int64_t slab = w.h_stage_doubles / per_prop;
+    e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * GW_NPARAM, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    for (int64_t b0 = 0; b0 < n_prop; b0 += slab) {
+        const int64_t nb = (n_prop - b0 < slab) ? n_prop - b0 : slab;
+        rc = gw_waveform_batch(ctx, nb, w.theta_stage + b0 * GW_NPARAM, w.h_stage, cuda_stream);
+        if (rc != GW_OK) return rc;
+        e = cudaMemcpyAsync(h_out_host + b0 * per_prop, w.h_stage, sizeof(double) * nb * per_prop,
+                            cudaMemcpyDeviceToHost, s);
+        if (e != cudaSuccess) return cuda_fail(ctx, e);
+    }
+    if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(ctx, e);
+    return GW_OK;
+}
+
+int gw_probe_fp64_fma_rate(int n_iter, double *fma_per_s, double *elapsed_ms, void *cuda_stream)
+{
+    if (n_iter < 1) return GW_ERR_INVALID_ARG;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return GW_ERR_CUDA;
+    if (prop.major != 10) return GW_ERR_ARCH;
+    return probe_fma_rate(n_iter, fma_per_s, elapsed_ms, (cudaStream_t)cuda_stream) == cudaSuccess ? GW_OK : GW_ERR_CUDA;
+}
+
+} // extern "C"

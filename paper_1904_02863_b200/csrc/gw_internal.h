@@ -1,0 +1,79 @@
+// gw_internal.h -- host-side structs shared by gw_api.cu (C-ABI + host logic) and gw_kernels.cu
+// (kernels + launchers).  Not part of the public boundary (include/gwlnl.h).  Shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/gwlnl.h"
+
+namespace gw {
+
+constexpr int kThreads    = 256;   // threads per CTA of the fused and waveform kernels
+constexpr int kStageBins  = 128;   // bins per shared-memory stage of the fused kernel
+constexpr int kStages     = 3;     // stage ring depth
+constexpr int kBasis      = 8;     // per-bin phase basis values (4 planes of 2)
+constexpr int kBasisPlanes = 4;
+constexpr int kRecFixed   = 10;    // record fields before the per-detector block
+constexpr int kRecPerDet  = 5;     // tau, Cre, Cim, rot_re, rot_im
+
+// One detector as the kernels see it (built on the host from gw_detector).
+struct DetGeom {
+    int    kind;          // GW_DET_GEOMETRIC | GW_DET_FIXED
+    double D[6];          // detector tensor (xx, xy, xz, yy, yz, zz) = (x(x)x - y(x)y)/2
+    double rc[3];         // vertex / c  [s]
+    double fplus, fcross, dt_s;
+};
+struct DetSet { DetGeom d[GW_MAX_DET]; };
+
+// Device tables of a context (all owned by the context).
+struct Tables {
+    int64_t n_bins;       // M
+    int64_t n_pad;        // allocated bins per plane (>= M, multiple of 32)
+    int     n_det;
+    double  f0, delta_f;
+    double *planes;       // [4 + n_det][n_pad][2]: basis planes (x^-5,x^-3) (x^-2,x^-1) (ln f,x) (x ln f,x^2), then g_I (re,im)
+    double *fm76;         // [n_pad]  f^(-7/6)
+    double *freq;         // [n_pad]  f_j
+    double  i7[GW_MAX_DET];   // host copy of I7_I = sum_j (4 df/S_Ij) f_j^(-7/3)
+};
+
+// Launch shape of one gw_lnl_batch call (a pure function of n_prop and the context; fixes summation order).
+struct Plan {
+    int     lpp;          // lanes per proposal (1,2,4,...,32)
+    int     props_per_cta;// kThreads / lpp
+    int     n_chunks;     // frequency chunks per proposal tile
+    int64_t n_tiles;      // ceil(n_prop / props_per_cta)
+};
+
+struct Workspace {
+    int64_t max_batch;    // reserved proposals
+    int64_t rec_stride;   // proposals per record field (>= max_batch, multiple of 32)
+    double *rec;          // [kRecFixed + kRecPerDet*n_det][rec_stride]
+    double *partial;      // chunk partials, size partial_doubles
+    int64_t partial_doubles;
+    unsigned int *tickets;// [max tiles]
+    int64_t n_tickets;
+    double *theta_stage;  // [max_batch][GW_NPARAM]   (host-variant staging)
+    double *lnl_stage;    // [max_batch]
+    double *parts_stage;  // [max_batch][n_det][3]
+    double *h_stage;      // waveform slab staging (host variant), h_stage_doubles
+    int64_t h_stage_doubles;
+};
+
+// ---- launchers (gw_kernels.cu).  All return the cudaError_t of the launch. ------------------------------
+cudaError_t launch_precompute(const Tables &t, const double *freqs_dev, const double *data_dev,
+                              const double *psd_dev, double *i7_dev, cudaStream_t s, int64_t *launches);
+cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int spin_order, int64_t n_prop,
+                         const double *theta_dev, double *rec, int64_t rec_stride, double rot_stride_hz,
+                         cudaStream_t s, int64_t *launches);
+cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, const double *rec,
+                         int64_t rec_stride, double *partial, unsigned int *tickets, double *lnl_out,
+                         double *parts_out, cudaStream_t s, int64_t *launches);
+cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, int64_t rec_stride,
+                            double *h_out, cudaStream_t s, int64_t *launches);
+cudaError_t configure_kernels(int *fused_ctas_per_sm);      // smem attributes + occupancy query (per n_det below)
+int         fused_ctas_per_sm(int n_det);
+size_t      fused_smem_bytes(int n_det);
+cudaError_t probe_fma_rate(int n_iter, double *fma_per_s, double *elapsed_ms, cudaStream_t s);
+
+} // namespace gw

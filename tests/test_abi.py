@@ -1,0 +1,88 @@
+"""`-m "not gpu"`: the C-ABI library builds for sm_100a, loads, and exports every symbol include/gwlnl.h
+declares; argument validation that needs no device; the product path fails loudly without a GPU."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1904_02863_b200.csrc import build as csrc_build
+    csrc_build.build()
+    from paper_1904_02863_b200 import binding
+    return binding.load_library()
+
+
+def _declared_functions():
+    text = open(os.path.join(ROOT, "include", "gwlnl.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(gw_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(lib):
+    from paper_1904_02863_b200 import binding
+    names = _declared_functions()
+    assert {"gw_ctx_create", "gw_waveform_batch", "gw_lnl_batch", "gw_ctx_destroy"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in gwlnl.h but not exported"
+    assert sorted(binding.EXPORTS) == names
+
+
+def test_no_compute_calls(lib):
+    assert lib.gw_abi_version() == 1
+    assert lib.gw_strerror(0) == b"ok" and b"invalid" in lib.gw_strerror(-1)
+    assert lib.gw_ctx_destroy(None) == 0
+    assert lib.gw_ctx_info(None, None, None, None, None) == -1
+    assert lib.gw_lnl_batch(None, 1, None, None, None, None) == -1
+    assert lib.gw_waveform_batch(None, 1, None, None, None) == -1
+    assert lib.gw_ctx_reserve(None, 8) == -1
+    assert lib.gw_last_cuda_error(None) == 0 and lib.gw_ctx_launch_count(None) == 0
+
+
+def test_create_rejects_bad_arguments_before_touching_cuda(lib):
+    from paper_1904_02863_b200 import binding
+    h = ctypes.c_void_p()
+    f = np.arange(20.0, 30.0, 0.25)
+    d = np.zeros((1, f.size, 2))
+    S = np.ones((1, f.size))
+    det = binding.detector_structs(np.array([[1, 0, 0, 0, 0, 0, 0, 0, 0, 0, 1, 0, 0.0]]))
+    fp, dp, sp = f.ctypes.data, d.ctypes.data, S.ctypes.data
+    assert lib.gw_ctx_create(None, f.size, fp, 1, dp, sp, det, 0.0, None, None) == binding.GW_ERR_INVALID_ARG
+    assert lib.gw_ctx_create(ctypes.byref(h), 1, fp, 1, dp, sp, det, 0.0, None, None) == binding.GW_ERR_INVALID_ARG
+    assert lib.gw_ctx_create(ctypes.byref(h), f.size, None, 1, dp, sp, det, 0.0, None, None) == binding.GW_ERR_INVALID_ARG
+    assert lib.gw_ctx_create(ctypes.byref(h), f.size, fp, 0, dp, sp, det, 0.0, None, None) == binding.GW_ERR_INVALID_ARG
+    assert lib.gw_ctx_create(ctypes.byref(h), f.size, fp, 5, dp, sp, det, 0.0, None, None) == binding.GW_ERR_INVALID_ARG
+    opt = binding.gw_options(1, 1, 16)      # isco_cut = 1 is not supported (A6)
+    assert lib.gw_ctx_create(ctypes.byref(h), f.size, fp, 1, dp, sp, det, 0.0, ctypes.byref(opt), None) == binding.GW_ERR_INVALID_ARG
+    assert not h
+
+
+def test_product_path_fails_loudly_without_gpu(lib):
+    """No CPU fallback: on a box without a CUDA device the context cannot be created (and nothing under
+    paper_1904_02863_b200 imports the oracle)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_1904_02863_b200 import binding
+    h = ctypes.c_void_p()
+    f = np.arange(20.0, 30.0, 0.25)
+    d = np.zeros((1, f.size, 2))
+    S = np.ones((1, f.size))
+    det = binding.detector_structs(np.array([[1, 0, 0, 0, 0, 0, 0, 0, 0, 0, 1, 0, 0.0]]))
+    rc = lib.gw_ctx_create(ctypes.byref(h), f.size, f.ctypes.data, 1, d.ctypes.data, S.ctypes.data, det, 0.0, None, None)
+    assert rc in (binding.GW_ERR_CUDA, binding.GW_ERR_ARCH) and not h
+
+
+def test_package_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_1904_02863_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, fn)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", text, flags=re.M), fn
+                assert "gw_oracle" not in text, fn

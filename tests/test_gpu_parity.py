@@ -1,0 +1,293 @@
+"""`-m gpu`: the CUDA path (through the C-ABI of include/gwlnl.h) against the CPU oracle, element by element,
+on the same seeded inputs (SURVEY.md section 9 gates 2-4; tolerances from BASELINE.json north_star)."""
+import numpy as np
+import pytest
+
+from paper_1904_02863_b200 import inputs
+
+from gpu_common import assert_h_close, assert_lnl_close, make_ctx, make_problem
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    return torch
+
+
+def _dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+# reduced shapes: several stages (128 bins) and chunks, ragged tails in bins and in proposals
+SMALL = [
+    ("C0", dict(f_max=512.0, batch=256)),          # config 0 at full size: 3937 bins, 256 proposals, 1 fixed det
+    ("C1", dict(f_max=181.75, batch=300)),         # 648 bins (5 stages + 8), 300 proposals (2 tiles, ragged)
+    ("C2", dict(f_max=24.5, batch=70)),            # BNS: 577 bins at df = 1/128, phases ~1e4 rad
+    ("C3", dict(f_max=11.25, batch=40)),           # 10 Hz start, df = 1/512: 641 bins, phases ~4.5e4 rad
+    ("C4", dict(f_max=2048.0, batch=48)),          # config-1 shape at full band (8113 bins)
+]
+
+
+@pytest.mark.parametrize("name,red", SMALL, ids=[s[0] for s in SMALL])
+def test_waveform_elementwise(oracle, torch_cuda, name, red):
+    torch = torch_cuda
+    cfg = inputs.CONFIGS[name].reduced(**red)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    nb = min(cfg.batch, 64)
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        h = ctx.waveform_batch(_dev(torch, th[:nb]))
+        torch.cuda.synchronize()
+        h_gpu = h.cpu().numpy()
+    h_ref = oracle.waveform(f, dets, cfg.gmst, th[:nb], cfg.spin_order)
+    assert h_gpu.shape == h_ref.shape
+    assert_h_close(h_gpu, h_ref)
+
+
+@pytest.mark.parametrize("name,red", SMALL, ids=[s[0] for s in SMALL])
+def test_lnl_every_proposal(oracle, torch_cuda, name, red):
+    torch = torch_cuda
+    cfg = inputs.CONFIGS[name].reduced(**red)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        lnl, parts = ctx.lnl_batch(_dev(torch, th), want_parts=True)
+        torch.cuda.synchronize()
+        lnl, parts = lnl.cpu().numpy(), parts.cpu().numpy()
+    lnl_ref, parts_ref, _ = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th, cfg.spin_order)
+    assert_lnl_close(lnl, parts, lnl_ref, parts_ref)
+    # row 0 is the injection: coherent, Re<d|h> ~ <h|h>
+    assert parts[0, :, 0].sum() == pytest.approx(parts[0, :, 2].sum(), rel=0.2)
+
+
+@pytest.mark.parametrize("batch", [1, 2, 3, 7, 8, 9, 16, 31, 33, 64, 100, 255, 257, 600])
+def test_lnl_all_lane_layouts(oracle, torch_cuda, batch):
+    """Every lanes-per-proposal layout of the fused kernel (1..32 lanes, ragged tiles) gives the oracle's lnL."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=301.25, batch=600)        # 1126 bins
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        plan = ctx.plan(batch)
+        lnl, parts = ctx.lnl_batch(_dev(torch, th[:batch]), want_parts=True)
+        torch.cuda.synchronize()
+        lnl, parts = lnl.cpu().numpy(), parts.cpu().numpy()
+    lnl_ref, parts_ref, _ = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:batch], cfg.spin_order)
+    assert_lnl_close(lnl, parts, lnl_ref, parts_ref)
+    assert plan["lanes_per_prop"] * plan["props_per_cta"] == 256
+
+
+def test_lane_layouts_cover_all_widths(oracle, torch_cuda):
+    """The planner reaches every lane width 1..32 somewhere in the sweep used above (so the test above covers them)."""
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=301.25, batch=600)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    seen = set()
+    with make_ctx(cfg, f, d, S, dets, max_batch=70000) as ctx:
+        for b in [1, 2, 3, 7, 8, 9, 16, 31, 33, 64, 100, 255, 257, 600, 4096, 70000]:
+            seen.add(ctx.plan(b)["lanes_per_prop"])
+    assert 1 in seen and 32 in seen and len(seen) >= 3, seen
+
+
+@pytest.mark.parametrize("n_det", [1, 2, 4])
+def test_detector_counts(oracle, torch_cuda, n_det):
+    """1, 2 and 4 detectors (mixed GEOMETRIC / FIXED with a non-zero fixed delay)."""
+    torch = torch_cuda
+    base = inputs.CONFIGS["C1"].reduced(f_max=150.0, batch=40)
+    rows = [inputs.geometric_detector("H1"), inputs.fixed_detector(0.6, -0.3, 0.0123),
+            inputs.geometric_detector("V1"), inputs.geometric_detector("L1")][:n_det]
+    dets = np.stack(rows)
+    f = inputs.frequency_grid(base)
+    S = np.tile(inputs.analytic_psd(f), (n_det, 1))
+    th = inputs.proposals(base)
+    rng = np.random.Generator(np.random.PCG64(777 + n_det))
+    z = rng.standard_normal((n_det, f.size, 2))
+    sig = oracle.waveform(f, dets, base.gmst, th[:1])[0]
+    d = sig + (z[..., 0] + 1j * z[..., 1]) * np.sqrt(S / (4 * base.delta_f))
+    from paper_1904_02863_b200 import GwContext
+    with GwContext(f, d, S, dets, base.gmst, max_batch=64) as ctx:
+        thd = _dev(torch, th)
+        lnl, parts = ctx.lnl_batch(thd, want_parts=True)
+        h = ctx.waveform_batch(thd)
+        torch.cuda.synchronize()
+        lnl, parts, h = lnl.cpu().numpy(), parts.cpu().numpy(), h.cpu().numpy()
+    lnl_ref, parts_ref, _ = oracle.lnl(f, base.delta_f, d, S, dets, base.gmst, th)
+    assert_lnl_close(lnl, parts, lnl_ref, parts_ref)
+    assert_h_close(h, oracle.waveform(f, dets, base.gmst, th))
+
+
+def test_precompute_norms(oracle, torch_cuda):
+    """Kernel K0: I7_I = sum (4 df/S) f^(-7/3) against the oracle's compensated sum; <h|h> = |C|^2 A0^2 I7 (pin P2)."""
+    for name, red in SMALL:
+        cfg = inputs.CONFIGS[name].reduced(**red)
+        f, S, dets = inputs.frequency_grid(cfg), inputs.psd(cfg), inputs.detectors(cfg)
+        with make_ctx(cfg, f, np.zeros_like(S, dtype=complex), S, dets) as ctx:
+            i7 = ctx.norms()
+        ref = oracle.norm_i7(f, cfg.delta_f, S[0])
+        np.testing.assert_allclose(i7, ref, rtol=1e-13)
+
+
+def test_no_spin_option(oracle, torch_cuda):
+    """spin_order = 0 ignores chi1, chi2 (config C0 is non-spinning)."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=120.0, batch=33)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    from paper_1904_02863_b200 import GwContext
+    with GwContext(f, d, S, dets, cfg.gmst, spin_order=0, max_batch=64) as ctx:
+        lnl, parts = ctx.lnl_batch(_dev(torch, th), want_parts=True)
+        torch.cuda.synchronize()
+    lnl_ref, parts_ref, _ = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th, spin_order=0)
+    assert_lnl_close(lnl.cpu().numpy(), parts.cpu().numpy(), lnl_ref, parts_ref)
+
+
+def test_bitwise_determinism_and_prefix_stability(oracle, torch_cuda):
+    """Gate 4: >= 10 repeats give identical bits; a proposal's lnL does not depend on what else shares the
+    batch as long as the launch shape (plan) is unchanged."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=420.0, batch=700)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        thd = _dev(torch, th)
+        first, first_parts = ctx.lnl_batch(thd, want_parts=True)
+        first, first_parts = first.clone(), first_parts.clone()
+        for _ in range(10):
+            again, again_parts = ctx.lnl_batch(thd, want_parts=True)
+            torch.cuda.synchronize()
+            assert torch.equal(again, first) and torch.equal(again_parts, first_parts)
+        # same plan (tile count and chunking) for 700 and 690 proposals => identical bits for the shared prefix
+        if ctx.plan(700) == ctx.plan(690):
+            sub = ctx.lnl_batch(thd[:690].contiguous())
+            torch.cuda.synchronize()
+            assert torch.equal(sub, first[:690])
+        # waveform: pure function of (theta_b, bin)
+        h1 = ctx.waveform_batch(thd[:50].contiguous()).clone()
+        h2 = ctx.waveform_batch(thd[10:60].contiguous())
+        torch.cuda.synchronize()
+        assert torch.equal(h1[10:], h2[:40])
+
+
+def test_host_variants_match_device_variants(oracle, torch_cuda):
+    torch = torch_cuda
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=200.0, batch=130)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        lnl_d, parts_d = ctx.lnl_batch(_dev(torch, th), want_parts=True)
+        h_d = ctx.waveform_batch(_dev(torch, th))
+        torch.cuda.synchronize()
+        lnl_h, parts_h = ctx.lnl_batch_host(th, want_parts=True)
+        h_h = ctx.waveform_batch_host(th)
+        lnl_only = ctx.lnl_batch_host(th)
+    assert np.array_equal(lnl_h, lnl_d.cpu().numpy()) and np.array_equal(parts_h, parts_d.cpu().numpy())
+    assert np.array_equal(h_h, h_d.cpu().numpy()) and np.array_equal(lnl_only, lnl_h)
+
+
+def test_device_resident_context_inputs(oracle, torch_cuda):
+    """gw_ctx_create accepts device pointers for freqs / data / psd."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=100.0, batch=20)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    from paper_1904_02863_b200 import GwContext
+    with GwContext(f, d, S, dets, cfg.gmst, max_batch=32) as a, \
+            GwContext(_dev(torch, f), _dev(torch, d), _dev(torch, S), dets, cfg.gmst, max_batch=32) as b:
+        la = a.lnl_batch(_dev(torch, th))
+        lb = b.lnl_batch(_dev(torch, th))
+        torch.cuda.synchronize()
+        assert torch.equal(la, lb)
+
+
+def test_identities_on_gpu(oracle, torch_cuda):
+    """Pin P3 through the CUDA path: d = 0 => lnL = -1/2 <h|h>; noiseless data at the truth => +1/2 <h|h>, Im<d|h> = 0."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=256.0, batch=64)
+    f, S, dets = inputs.frequency_grid(cfg), inputs.psd(cfg), inputs.detectors(cfg)
+    th = inputs.proposals(cfg)
+    with make_ctx(cfg, f, np.zeros_like(S, dtype=complex), S, dets) as ctx:
+        lnl, parts = ctx.lnl_batch(_dev(torch, th), want_parts=True)
+        torch.cuda.synchronize()
+        lnl, parts = lnl.cpu().numpy(), parts.cpu().numpy()
+        assert np.all(parts[..., :2] == 0)
+        np.testing.assert_allclose(lnl, -0.5 * parts[..., 2].sum(axis=1), rtol=1e-14)
+        sig = ctx.waveform_batch(_dev(torch, th[:1]))[0].cpu().numpy()      # the library's own h as data
+    with make_ctx(cfg, f, sig, S, dets) as ctx:
+        lnl, parts = ctx.lnl_batch(_dev(torch, th), want_parts=True)
+        torch.cuda.synchronize()
+        lnl, parts = lnl.cpu().numpy(), parts.cpu().numpy()
+    hh = parts[0, :, 2].sum()
+    assert lnl[0] == pytest.approx(0.5 * hh, rel=1e-10)
+    assert np.abs(parts[0, :, 1]).max() < 1e-9 * hh
+    assert np.all(lnl[1:] < 0.5 * hh)                                       # Cauchy-Schwarz
+
+
+def test_edge_cases_and_errors(oracle, torch_cuda):
+    torch = torch_cuda
+    from paper_1904_02863_b200 import GwContext, GwError
+    from paper_1904_02863_b200 import binding
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=60.0, batch=16)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    with GwContext(f, d, S, dets, cfg.gmst, max_batch=16) as ctx:
+        # n_prop == 0: OK, writes nothing
+        empty = torch.empty((0, 11), dtype=torch.float64, device="cuda")
+        out = ctx.lnl_batch(empty)
+        assert out.numel() == 0
+        assert ctx.waveform_batch(empty).shape == (0, 3, f.size)
+        # more than reserved: INVALID_ARG, then reserve and retry
+        big = _dev(torch, np.tile(th, (2, 1)))
+        with pytest.raises(GwError) as ei:
+            ctx.lnl_batch(big)
+        assert ei.value.code == binding.GW_ERR_INVALID_ARG
+        ctx.reserve(32)
+        assert ctx.info()["max_batch"] == 32
+        both = ctx.lnl_batch(big)
+        torch.cuda.synchronize()
+        assert torch.equal(both[:16], both[16:])
+        # out-of-domain rows give NaN there and nowhere else
+        bad = th.copy()
+        bad[3, inputs.P_MC] = -1.0
+        bad[5, inputs.P_Q] = 1.5
+        bad[7, inputs.P_DL] = 0.0
+        bad[9, inputs.P_COSI] = 1.2
+        bad[11, inputs.P_TC] = np.nan
+        lnl, parts = ctx.lnl_batch(_dev(torch, bad), want_parts=True)
+        h = ctx.waveform_batch(_dev(torch, bad))
+        good = ctx.lnl_batch(_dev(torch, th))
+        torch.cuda.synchronize()
+        lnl, h, good = lnl.cpu().numpy(), h.cpu().numpy(), good.cpu().numpy()
+        rows = [3, 5, 7, 9, 11]
+        assert np.all(np.isnan(lnl[rows])) and np.all(np.isnan(h[rows]))
+        keep = np.setdiff1d(np.arange(16), rows)
+        assert np.array_equal(lnl[keep], good[keep]) and np.all(np.isfinite(h[keep]))
+    # smallest grid: 2 bins
+    f2, S2 = f[:2], S[:, :2]
+    with GwContext(f2, d[:, :2], S2, dets, cfg.gmst, max_batch=16) as ctx:
+        lnl = ctx.lnl_batch_host(th)
+    ref, _, _ = oracle.lnl(f2, cfg.delta_f, d[:, :2], S2, dets, cfg.gmst, th)
+    np.testing.assert_allclose(lnl, ref, rtol=1e-9, atol=1e-12)
+    # create-time validation
+    fbad = f.copy(); fbad[5] += 1e-3
+    for args in [(fbad, d, S), (f, d, -S), (f[::-1].copy(), d, S)]:
+        with pytest.raises(GwError) as ei:
+            GwContext(args[0], args[1], args[2], dets, cfg.gmst)
+        assert ei.value.code == binding.GW_ERR_INVALID_ARG
+    skew = dets.copy(); skew[0, 4:7] *= 1.01
+    with pytest.raises(GwError):
+        GwContext(f, d, S, skew, cfg.gmst)
+    with pytest.raises(GwError):
+        GwContext(f, d[:2], S[:2], np.tile(dets[:1], (5, 1)), cfg.gmst)      # 5 detectors > GW_MAX_DET
+
+
+def test_time_shift_interchange(oracle, torch_cuda):
+    """Pin P4 on the GPU: a FIXED detector with dt = tau is the same as t_c + tau (PAPER.md:69 factor)."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS["C0"].reduced(f_max=128.0, batch=32)
+    f, S = inputs.frequency_grid(cfg), inputs.psd(cfg)
+    th = inputs.proposals(cfg)
+    tau = 0.0123
+    from paper_1904_02863_b200 import GwContext
+    zero = np.zeros_like(S, dtype=complex)
+    with GwContext(f, zero, S, inputs.fixed_detector(1.0, 0.0, tau)[None], 0.0, spin_order=0, max_batch=32) as a, \
+            GwContext(f, zero, S, inputs.fixed_detector(1.0, 0.0, 0.0)[None], 0.0, spin_order=0, max_batch=32) as b:
+        th2 = th.copy(); th2[:, inputs.P_TC] += tau
+        ha = a.waveform_batch_host(th)
+        hb = b.waveform_batch_host(th2)
+    scale = np.abs(hb).max(axis=-1, keepdims=True)
+    assert (np.abs(ha - hb) / scale).max() < 1e-11
+    np.testing.assert_allclose(np.abs(ha), np.abs(hb), rtol=1e-12)
