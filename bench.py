@@ -1,0 +1,351 @@
+#!/usr/bin/env python3
+"""bench.py -- likelihood evaluations/s of the fused waveform+lnL hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic proposals: gw_lnl_batch = setup kernel
+(K1) + fused kernel (K3) on the workload's full batch.  The default workload is BASELINE.json configs[1]
+(C1: 3 detectors, 8113 bins, 4096 proposals); --workload C0|C2|C3|C4:<B> runs the others (parity-test cases).
+Inputs are seeded and synthetic (paper_1904_02863_b200/inputs.py); the injection is computed with the library's
+own gw_waveform_batch, so the product arm never touches oracle/.
+
+Timing: per-step CUDA events on the launching stream, L2 flushed (a 256 MiB write) before every timed step,
+>= 3 warm-up steps after a clock ramp, clocks sampled through NVML during the timed region.  N > 1: one process
+per GPU under torchrun, proposals sharded with no collective on the data path (weak scaling); NCCL carries only
+the barrier and the max-over-ranks reduction of the measured time.
+
+--impl reference times the CPU oracle (oracle/, plain C, fp64) on the host cores on a bounded sample of the
+same workload; it is the one place besides `cpu_baseline` where bench.py executes oracle/.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "likelihood evals/sec (fp64, waveform+lnL)"
+UNIT = "lnL/s"
+FP64_LANES_PER_SM = 64          # B200 fp64 FMA lanes per SM (37.2 TFLOP/s at 1965 MHz x 148 SMs)
+L2_FLUSH_BYTES = 256 << 20
+
+
+def parse_workload(spec):
+    from paper_1904_02863_b200 import inputs
+    name, _, b = spec.partition(":")
+    cfg = inputs.CONFIGS[name]
+    batch = int(b) if b else (4096 if name == "C4" else cfg.batch)
+    return name, cfg, batch
+
+
+def walg_per_bin(n_det):
+    """Algorithmic fp64 FMA-equivalents per (proposal, bin): SURVEY.md 8(d) W_alg = 31 + 8 N_det."""
+    return 31 + 8 * n_det
+
+
+class ClockSampler:
+    """NVML clock / throttle-reason samples during the timed region (a thread; ~2 ms cadence)."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:          # no NVML: report that, do not invent numbers
+            self.nv, self.err = None, repr(e)
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": nv.nvmlClocksEventReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksEventReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksEventReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksEventReasonSwPowerCap}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+
+    def summary(self):
+        if self.nv is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable: " + self.err]}
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def build_problem(cfg, batch_total):
+    """freqs, data, psd, det rows, theta[batch_total] -- the injection comes from the library's own waveform."""
+    from dataclasses import replace
+    from paper_1904_02863_b200 import binding, inputs
+    f = inputs.frequency_grid(cfg)
+    S = inputs.psd(cfg)
+    dets = inputs.detectors(cfg)
+    d = inputs.make_data(cfg, binding.waveform_for_inputs)
+    draw = max(cfg.batch, batch_total)
+    th = inputs.proposals(replace(cfg, batch=draw))[:batch_total]
+    return f, S, dets, d, th
+
+
+def oracle_rate(cfg, f, S, dets, d, th, target_s, n_threads=0):
+    """Time the oracle, as it stands, on a bounded prefix of the proposals (~target_s of CPU work)."""
+    import oracle
+    oracle.build()
+    pilot = th[: min(len(th), max(2, os.cpu_count() or 1))]
+    t0 = time.perf_counter()
+    _, _, used = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, pilot, cfg.spin_order, n_threads)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    n = int(min(len(th), max(len(pilot), len(pilot) * target_s / dt)))
+    t0 = time.perf_counter()
+    _, _, used = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order, n_threads)
+    dt = time.perf_counter() - t0
+    return n / dt, used, n, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    name, cfg, batch = parse_workload(args.workload)
+    import oracle
+    oracle.build()
+    from paper_1904_02863_b200 import inputs
+    f, S, dets = inputs.frequency_grid(cfg), inputs.psd(cfg), inputs.detectors(cfg)
+    d = inputs.make_data(cfg, oracle.waveform)
+    th = inputs.proposals(cfg)[:batch] if batch <= cfg.batch else inputs.proposals(cfg)
+    # size one step to ~ (90 s budget) / (steps + warmup)
+    per_step_s = min(10.0, 90.0 / max(1, args.steps + args.warmup))
+    rate, used, n, _ = oracle_rate(cfg, f, S, dets, d, th, per_step_s)
+    n = max(1, min(len(th), int(rate * per_step_s)))
+    for _ in range(args.warmup):
+        oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _, _, used = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order)
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    sample = f"first {n} of {batch} proposals of {name} per step, all {cfg.n_bins} bins x {cfg.n_det} detectors"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{name}: {cfg.n_det} det x {cfg.n_bins} bins x {batch} proposals per GPU",
+                       "global_batch": batch, "bins": cfg.n_bins, "detectors": cfg.n_det},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1904_02863_b200.csrc import build as csrc_build
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0 and os.path.exists(csrc_build.NVCC):
+        csrc_build.build()             # no-op when csrc/libgwlnl.so is newer than its sources
+    from paper_1904_02863_b200 import GwContext, binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    n_gpus = world
+
+    name, cfg, batch = parse_workload(args.workload)
+    f, S, dets, d, th_all = build_problem(cfg, batch * world)
+    from paper_1904_02863_b200.sharding import shard_range
+    lo, hi = shard_range(batch * world, rank, world)
+    th = np.ascontiguousarray(th_all[lo:hi])
+    B, M, n_det = len(th), cfg.n_bins, cfg.n_det
+    stream = torch.cuda.current_stream()
+
+    ctx = GwContext(f, d, S, dets, cfg.gmst, spin_order=cfg.spin_order, max_batch=B)
+    thd = torch.from_numpy(th).cuda()
+    lnl = torch.empty(B, dtype=torch.float64, device="cuda")
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+    plan = ctx.plan(B)
+
+    # ---- clock ramp + measured fp64 FMA rate (the measured roofline denominator) ----
+    fma_rate, _ = binding.probe_fp64_fma_rate(1 << 14)
+    fma_rate, _ = binding.probe_fp64_fma_rate(1 << 15)
+
+    def step():
+        ctx.lnl_batch(thd, out=lnl)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+
+    # ---- timed region: K steps, per-step events, L2 flush before each ----
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    launches0 = ctx.launch_count()
+    with ClockSampler(local) as clk:
+        for i in range(args.steps):
+            flush.fill_(i & 0xff)
+            ev0[i].record(stream)
+            step()
+            ev1[i].record(stream)
+        torch.cuda.synchronize()
+    launches = ctx.launch_count() - launches0
+    if world > 1:
+        dist.barrier()
+    step_ms = np.array([a.elapsed_time(b) for a, b in zip(ev0, ev1)])
+    total_ms = float(step_ms.sum())
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    value = B * world * args.steps / (total_ms * 1e-3)
+
+    # ---- kernel-level pass (same stream, events inside the library around K3), flushed likewise ----
+    ctx.kernel_timing(True)
+    k_ms, s_ms = [], []
+    for i in range(args.steps):
+        flush.fill_(i & 0xff)
+        step()
+        a, b = ctx.last_kernel_ms()
+        s_ms.append(a)
+        k_ms.append(b)
+    ctx.kernel_timing(False)
+    fused_ms = float(np.mean(k_ms))
+    walg = walg_per_bin(n_det)
+    flops_per_launch = 2.0 * walg * B * M
+    achieved = flops_per_launch / (fused_ms * 1e-3) / 1e12
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    peak = n_sm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    roofline = {"bound": "alu", "kernel": "fused_kernel<%d>" % n_det, "achieved": achieved, "peak": peak,
+                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                "peak_source": "derived: %d SMs x %d fp64 FMA lanes x 2 flop x %.0f MHz (MEASURED_PEAKS sm_max_mhz)"
+                               % (n_sm, FP64_LANES_PER_SM, sm_max),
+                "peak_measured_fma_probe": 2 * fma_rate / 1e12, "frac_of_measured": achieved / (2 * fma_rate / 1e12),
+                "flop_per_launch": flops_per_launch, "walg_fma_per_prop_bin": walg,
+                "kernel_ms": fused_ms, "setup_kernel_ms": float(np.mean(s_ms))}
+
+    # ---- end to end: host buffers through gw_lnl_batch_host (H2D + kernels + D2H + sync inside the call) ----
+    th_pin = torch.from_numpy(th).pin_memory()
+    out_pin = torch.empty(B, dtype=torch.float64).pin_memory()
+    th_host, out_host = th_pin.numpy(), out_pin.numpy()
+    for _ in range(3):
+        ctx.lnl_batch_host(th_host, out=out_host)
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ctx.lnl_batch_host(th_host, out=out_host)
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = {"value": B * world * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(th.nbytes) * world,
+           "d2h_bytes_per_step": int(out_host.nbytes) * world, "ms_per_step": 1e3 * e2e_s / args.steps,
+           "api": "gw_lnl_batch_host (pinned host theta in, host lnL out, stream synchronised)"}
+
+    # ---- the waveform-only kernel (north_star item (3)): achieved HBM GB/s ----
+    extra = {}
+    if rank == 0 and not args.no_waveform:
+        wb = min(B, max(1, int((2 << 30) // (n_det * M * 16))))
+        h = torch.empty((wb, n_det, M), dtype=torch.complex128, device="cuda")
+        thw = thd[:wb].contiguous()
+        for _ in range(3):
+            ctx.waveform_batch(thw, out=h)
+        ctx.kernel_timing(True)
+        w_ms = []
+        for i in range(max(3, min(args.steps, 10))):
+            flush.fill_(i & 0xff)
+            ctx.waveform_batch(thw, out=h)
+            w_ms.append(ctx.last_kernel_ms()[1])
+        ctx.kernel_timing(False)
+        gbs = wb * n_det * M * 16 / (np.mean(w_ms) * 1e-3) / 1e9
+        hbm = float(peaks.get("hbm_gbs", 6650.0))
+        extra["waveform_kernel"] = {"proposals": wb, "bytes_stored": wb * n_det * M * 16, "kernel_ms": float(np.mean(w_ms)),
+                                    "achieved_GBps": gbs, "hbm_peak_GBps": hbm,
+                                    "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback",
+                                    "frac": gbs / hbm}
+        del h
+
+    # ---- CPU baseline: the oracle as it stands on this box's host cores (rank 0, N = 1 only) ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        rate, used, n, dt = oracle_rate(cfg, f, S, dets, d, th, args.cpu_seconds)
+        cpu = {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle",
+               "sample": f"first {n} of {B} proposals, all {M} bins x {n_det} detectors, {dt:.1f} s"}
+
+    clocks = clk.summary()
+    ctx.close()
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n_gpus, "steps": args.steps,
+                "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"{name}: {n_det} det x {M} bins x {B} proposals per GPU",
+                           "global_batch": B * world, "bins": M, "detectors": n_det, "parallelism": f"proposals sharded x{world}",
+                           "l2": "flushed (256 MiB write) before every timed step", "plan": plan},
+                "bin_det_proposals_per_s": value * M * n_det,
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+                "roofline": roofline, "cpu_baseline": cpu}
+        line.update(extra)
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C1")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-waveform", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -94,7 +94,8 @@ typedef struct gw_ctx gw_ctx;    /* opaque */
  * per-detector norm I7 = sum_f (4 df/S) f^(-7/3).  Synchronises `cuda_stream` before returning.
  *   out        receives the context (set to NULL on error)
  *   n_bins     M >= 2
- *   freqs_hz   [M] host or dev; strictly positive, ascending, uniform (|f_j - f_0 - j df| <= 1e-6 df);
+ *   freqs_hz   [M] host or dev; strictly positive, ascending, uniform to rounding
+ *              (|f_j - f_0 - j df| <= 1e-9 df + 8 ulp(f_max): the time shift is applied by a recurrence on the grid);
  *              df is taken as (f[M-1] - f[0])/(M-1)
  *   n_det      1..GW_MAX_DET
  *   data_ri    [n_det][M][2] host or dev; one-sided continuous-normalised transform d(f), strain/Hz, finite
@@ -130,7 +131,7 @@ int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *l
 /* Host-buffer variants: theta_host -> (ctx-owned device staging) -> kernels -> outputs copied back to
  * host; the stream is synchronised before returning.  Pinned host memory makes the copies asynchronous
  * with respect to the host but is not required.  The waveform variant processes the batch in slabs
- * that fit the staging buffer reserved at create/reserve time.                                          */
+ * of at most 512 MiB through a device staging buffer it allocates on first use.                                          */
 int gw_lnl_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, double *lnl_out_host,
                       double *parts_out_host, void *cuda_stream);
 int gw_waveform_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, double *h_out_host,
@@ -152,6 +153,13 @@ int gw_ctx_norms(const gw_ctx *ctx, double *i7_host);
 
 /* Number of kernel launches the library has enqueued through this context so far.                      */
 int64_t gw_ctx_launch_count(const gw_ctx *ctx);
+
+/* Measurement aid: when enabled, the *_batch calls record CUDA events on their stream before the setup
+ * kernel, between the setup kernel and the main (fused or waveform) kernel, and after it.  The event between
+ * the two launches removes their programmatic overlap, so enable it only for kernel-level timing.
+ * gw_ctx_last_kernel_ms waits for the most recent call and returns the two durations.                  */
+int gw_ctx_kernel_timing(gw_ctx *ctx, int enable);
+int gw_ctx_last_kernel_ms(gw_ctx *ctx, double *setup_ms, double *main_ms);
 
 /* Register-resident dependent-FMA microbenchmark on the current device: enqueues `n_iter` rounds and
  * reports achieved fp64 FMA/s (the measured roofline denominator; MEASURED_PEAKS.json has no fp64

@@ -24,7 +24,7 @@ GW_OK, GW_ERR_INVALID_ARG, GW_ERR_ALLOC, GW_ERR_CUDA, GW_ERR_ARCH = 0, -1, -2, -
 EXPORTS = (
     "gw_ctx_create", "gw_ctx_reserve", "gw_waveform_batch", "gw_lnl_batch", "gw_lnl_batch_host",
     "gw_waveform_batch_host", "gw_ctx_destroy", "gw_ctx_info", "gw_ctx_plan", "gw_ctx_norms",
-    "gw_ctx_launch_count", "gw_probe_fp64_fma_rate", "gw_strerror", "gw_last_cuda_error", "gw_abi_version",
+    "gw_ctx_launch_count", "gw_ctx_kernel_timing", "gw_ctx_last_kernel_ms", "gw_probe_fp64_fma_rate", "gw_strerror", "gw_last_cuda_error", "gw_abi_version",
 )
 
 
@@ -76,6 +76,8 @@ def load_library():
     lib.gw_ctx_norms.argtypes = [vp, P(dbl)]
     lib.gw_ctx_launch_count.argtypes = [vp]
     lib.gw_ctx_launch_count.restype = i64
+    lib.gw_ctx_kernel_timing.argtypes = [vp, ci]
+    lib.gw_ctx_last_kernel_ms.argtypes = [vp, P(dbl), P(dbl)]
     lib.gw_probe_fp64_fma_rate.argtypes = [ci, P(dbl), P(dbl), vp]
     lib.gw_strerror.argtypes = [ci]
     lib.gw_strerror.restype = ctypes.c_char_p
@@ -206,6 +208,15 @@ class GwContext:
 
     def launch_count(self) -> int:
         return int(self._lib.gw_ctx_launch_count(self._h))
+
+    def kernel_timing(self, enable: bool):
+        _check(self._lib.gw_ctx_kernel_timing(self._h, int(bool(enable))), "gw_ctx_kernel_timing", self._h)
+
+    def last_kernel_ms(self):
+        """(setup kernel ms, main kernel ms) of the most recent *_batch call made with kernel_timing(True)."""
+        a, b = ctypes.c_double(), ctypes.c_double()
+        _check(self._lib.gw_ctx_last_kernel_ms(self._h, ctypes.byref(a), ctypes.byref(b)), "gw_ctx_last_kernel_ms", self._h)
+        return a.value, b.value
 
     def reserve(self, max_batch: int):
         _check(self._lib.gw_ctx_reserve(self._h, int(max_batch)), "gw_ctx_reserve", self._h)

@@ -22,6 +22,8 @@ struct gw_ctx {
     Workspace    w;
     int          last_cuda_error;
     int64_t      launches;
+    int          timing;           // gw_ctx_kernel_timing: record events around K1 and the main kernel
+    cudaEvent_t  ev[3];            // before K1, between K1 and main, after main
 };
 
 namespace {
@@ -299,6 +301,7 @@ int gw_ctx_destroy(gw_ctx *ctx)
     cudaDeviceSynchronize();
     free_workspace(ctx->w);
     cudaFree(ctx->t.planes); cudaFree(ctx->t.fm76); cudaFree(ctx->t.freq);
+    for (int i = 0; i < 3; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
     cudaGetLastError();
     return GW_OK;
@@ -335,6 +338,32 @@ int gw_ctx_norms(const gw_ctx *ctx, double *i7_host)
 
 int64_t gw_ctx_launch_count(const gw_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
+int gw_ctx_kernel_timing(gw_ctx *ctx, int enable)
+{
+    if (!ctx) return GW_ERR_INVALID_ARG;
+    if (enable && !ctx->ev[0]) {
+        for (int i = 0; i < 3; ++i) {
+            cudaError_t e = cudaEventCreate(&ctx->ev[i]);
+            if (e != cudaSuccess) return cuda_fail(ctx, e);
+        }
+    }
+    ctx->timing = enable ? 1 : 0;
+    return GW_OK;
+}
+
+int gw_ctx_last_kernel_ms(gw_ctx *ctx, double *setup_ms, double *main_ms)
+{
+    if (!ctx || !ctx->ev[0]) return GW_ERR_INVALID_ARG;
+    cudaError_t e = cudaEventSynchronize(ctx->ev[2]);
+    if (e != cudaSuccess) return cuda_fail(ctx, e);
+    float a = 0.f, b = 0.f;
+    if ((e = cudaEventElapsedTime(&a, ctx->ev[0], ctx->ev[1])) != cudaSuccess) return cuda_fail(ctx, e);
+    if ((e = cudaEventElapsedTime(&b, ctx->ev[1], ctx->ev[2])) != cudaSuccess) return cuda_fail(ctx, e);
+    if (setup_ms) *setup_ms = a;
+    if (main_ms) *main_ms = b;
+    return GW_OK;
+}
+
 int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *lnl_out_dev,
                  double *parts_out_dev, void *cuda_stream)
 {
@@ -343,12 +372,15 @@ int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *l
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Plan p = make_plan(ctx, n_prop);
     if (partial_need(ctx, p) > ctx->w.partial_doubles || p.n_tiles > ctx->w.n_tickets) return GW_ERR_INVALID_ARG;
+    if (ctx->timing) cudaEventRecord(ctx->ev[0], s);
     cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
                                  ctx->w.rec_stride, (double)p.lpp * ctx->t.delta_f, s, &ctx->launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
+    if (ctx->timing) cudaEventRecord(ctx->ev[1], s);
     e = launch_fused(ctx->t, p, n_prop, ctx->w.rec, ctx->w.rec_stride, ctx->w.partial, ctx->w.tickets, lnl_out_dev,
                      parts_out_dev, s, &ctx->launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
+    if (ctx->timing) cudaEventRecord(ctx->ev[2], s);
     return GW_OK;
 }
 
@@ -358,11 +390,14 @@ int gw_waveform_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, doub
     if (rc != GW_OK || n_prop == 0) return rc;
     if (((uintptr_t)h_out_dev & 15u) != 0) return GW_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (ctx->timing) cudaEventRecord(ctx->ev[0], s);
     cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
                                  ctx->w.rec_stride, ctx->t.delta_f, s, &ctx->launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
+    if (ctx->timing) cudaEventRecord(ctx->ev[1], s);
     e = launch_waveform(ctx->t, n_prop, ctx->w.rec, ctx->w.rec_stride, h_out_dev, s, &ctx->launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
+    if (ctx->timing) cudaEventRecord(ctx->ev[2], s);
     return GW_OK;
 }
 
