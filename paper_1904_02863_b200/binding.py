@@ -45,7 +45,8 @@ class gw_options(ctypes.Structure):
 
 
 def lib_path() -> str:
-    return os.path.join(_HERE, "csrc", "libgwlnl.so")
+    """csrc/libgwlnl.so, or the file named by $GWLNL_LIBRARY (a differently tuned build of the same sources)."""
+    return os.environ.get("GWLNL_LIBRARY") or os.path.join(_HERE, "csrc", "libgwlnl.so")
 
 
 _lib = None

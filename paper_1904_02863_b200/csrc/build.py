@@ -29,12 +29,13 @@ def up_to_date() -> bool:
     return all(os.path.getmtime(d) <= t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and up_to_date():
+def build(force: bool = False, verbose: bool = False, defines=(), out: str = LIB) -> str:
+    """defines: e.g. ("GW_THREADS=128",) for a tuning variant written to `out` (the default build has none)."""
+    if not force and out == LIB and not defines and up_to_date():
         return LIB
-    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
+    cmd = [NVCC] + FLAGS + [f"-D{d}" for d in defines] + (["-Xptxas", "-v"] if verbose else []) + ["-o", out] + SOURCES
     subprocess.run(cmd, check=True, cwd=HERE)
-    return LIB
+    return out
 
 
 if __name__ == "__main__":

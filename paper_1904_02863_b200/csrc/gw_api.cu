@@ -116,7 +116,7 @@ int reserve_impl(gw_ctx *ctx, int64_t max_batch)
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     const int64_t need_partial = partial_bound(ctx, max_batch);
-    const int64_t need_tickets = (max_batch + 7) / 8 + 1;     // tiles at lpp = 32
+    const int64_t need_tickets = max_batch / (kThreads / 32) + 2;   // tiles at lpp = 32
     Workspace w;
     std::memset(&w, 0, sizeof(w));
     w.max_batch = max_batch;

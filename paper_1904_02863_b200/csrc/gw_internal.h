@@ -8,9 +8,27 @@
 
 namespace gw {
 
-constexpr int kThreads    = 256;   // threads per CTA of the fused and waveform kernels
-constexpr int kStageBins  = 128;   // bins per shared-memory stage of the fused kernel
-constexpr int kStages     = 3;     // stage ring depth
+// Tunables (compile-time; build.py may override them with -D for sweeps).
+#ifndef GW_THREADS
+#define GW_THREADS 256
+#endif
+#ifndef GW_MIN_CTAS
+#define GW_MIN_CTAS 2
+#endif
+#ifndef GW_UNROLL
+#define GW_UNROLL 4
+#endif
+#ifndef GW_STAGE_BINS
+#define GW_STAGE_BINS 128
+#endif
+#ifndef GW_STAGES
+#define GW_STAGES 3
+#endif
+constexpr int kThreads    = GW_THREADS;     // threads per CTA of the fused and waveform kernels
+constexpr int kMinCtas    = GW_MIN_CTAS;    // __launch_bounds__ residency target of the fused kernel
+constexpr int kStageBins  = GW_STAGE_BINS;  // bins per shared-memory stage of the fused kernel
+constexpr int kStages     = GW_STAGES;      // stage ring depth
+constexpr int kUnroll     = GW_UNROLL;      // bins per unrolled trip of the fused hot loop
 constexpr int kBasis      = 8;     // per-bin phase basis values (4 planes of 2)
 constexpr int kBasisPlanes = 4;
 constexpr int kRecFixed   = 10;    // record fields before the per-detector block

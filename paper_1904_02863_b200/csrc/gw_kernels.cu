@@ -381,7 +381,7 @@ __device__ __forceinline__ void finish_proposal(const FusedArgs &a, int64_t b, c
 }
 
 template <int NDET, bool MULTI>
-__global__ void __launch_bounds__(kThreads, 2) fused_kernel(const FusedArgs a)
+__global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedArgs a)
 {
     constexpr int NP = kBasisPlanes + NDET;                  // planes per stage
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -444,8 +444,62 @@ __global__ void __launch_bounds__(kThreads, 2) fused_kernel(const FusedArgs a)
         mbar_wait(&bars[buf], (uint32_t)((s / kStages) & 1));
         const double2 *P = sm + (size_t)buf * NP * kStageBins;
         const int iters = MULTI ? (cnt + lpp - 1) / lpp : cnt;
-#pragma unroll 2
-        for (int it = 0; it < iters; ++it) {
+        int it = 0;
+        if (!MULTI) {
+            // kUnroll bins per trip, written plane by plane ("k-major"): consecutive fp64 instructions then
+            // share a register operand in the same slot (the coefficient across bins, c/s across detectors,
+            // z across the re/im pair), which the operand-reuse cache serves.  A DFMA with three fresh
+            // register operands issues at 2/3 rate on B200 (profiles/dfma_operand_probe).
+            for (; it + kUnroll <= iters; it += kUnroll) {
+                double ph[kUnroll], cs[kUnroll], sn[kUnroll];
+                {
+                    double2 v[kUnroll];
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) v[u] = P[0 * kStageBins + it + u];
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.c0, v[u].x, k.c5);
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.c2, v[u].y, ph[u]);
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) v[u] = P[1 * kStageBins + it + u];
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.c3, v[u].x, ph[u]);
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.c4, v[u].y, ph[u]);
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) v[u] = P[2 * kStageBins + it + u];
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.cL5, v[u].x, ph[u]);
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.c6, v[u].y, ph[u]);
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) v[u] = P[3 * kStageBins + it + u];
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.cL6, v[u].x, ph[u]);
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.c7, v[u].y, ph[u]);
+                }
+#pragma unroll
+                for (int u = 0; u < kUnroll; ++u) cis_turns(ph[u], cs[u], sn[u]);
+#pragma unroll
+                for (int u = 0; u < kUnroll; ++u) {              // bins in ascending order: the Z recurrence
+#pragma unroll
+                    for (int i = 0; i < NDET; ++i) {
+                        const double2 g = P[(kBasisPlanes + i) * kStageBins + it + u];
+                        const double t1 = g.y * sn[u];
+                        const double t2 = g.y * cs[u];
+                        const double a2 = __fma_rn(g.x, cs[u], -t1);          // Re g e^{+i 2 pi Phi'}
+                        const double b2 = __fma_rn(g.x, sn[u], t2);           // Im
+                        const double a3 = __fma_rn(zi[i], -ri_[i], a2);
+                        const double b3 = __fma_rn(zi[i], rr[i], b2);
+                        const double nr = __fma_rn(zr[i], rr[i], a3);
+                        const double ni = __fma_rn(zr[i], ri_[i], b3);
+                        zr[i] = nr; zi[i] = ni;
+                    }
+                }
+            }
+        }
+        for (; it < iters; ++it) {
             int jj = MULTI ? sub + it * lpp : it;
             bool masked = false;
             if (MULTI) { masked = jj >= cnt; jj = masked ? cnt - 1 : jj; }
