@@ -161,10 +161,13 @@ int64_t gw_ctx_launch_count(const gw_ctx *ctx);
 int gw_ctx_kernel_timing(gw_ctx *ctx, int enable);
 int gw_ctx_last_kernel_ms(gw_ctx *ctx, double *setup_ms, double *main_ms);
 
-/* Register-resident dependent-FMA microbenchmark on the current device: enqueues `n_iter` rounds and
- * reports achieved fp64 FMA/s (the measured roofline denominator; MEASURED_PEAKS.json has no fp64
- * entry).  Synchronises.  Returns GW_ERR_CUDA / GW_ERR_ARCH on failure.                                 */
-int gw_probe_fp64_fma_rate(int n_iter, double *fma_per_s, double *elapsed_ms, void *cuda_stream);
+/* Register-resident fp64 rate microbenchmark on the current device (8 independent chains per thread, 64 warps
+ * per SM): enqueues `n_iter` rounds of 64 instructions per thread and reports achieved fp64 FMA/s -- the measured
+ * roofline denominator (MEASURED_PEAKS.json has no fp64 entry).  `mode` selects the operand pattern:
+ * 0 = fma(v, imm, imm) (pipe peak); 1 = fma(a, b, v) with three distinct register operands; 2 = three register
+ * operands of which one is shared by consecutive instructions; 3 = mma.sync m8n8k4 f64.  Synchronises.
+ * Errors: GW_ERR_INVALID_ARG, GW_ERR_CUDA, GW_ERR_ARCH.                                                 */
+int gw_probe_fp64_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, void *cuda_stream);
 
 const char *gw_strerror(int code);
 int gw_last_cuda_error(const gw_ctx *ctx);      /* a cudaError_t value, 0 if none                         */

@@ -79,7 +79,7 @@ def load_library():
     lib.gw_ctx_launch_count.restype = i64
     lib.gw_ctx_kernel_timing.argtypes = [vp, ci]
     lib.gw_ctx_last_kernel_ms.argtypes = [vp, P(dbl), P(dbl)]
-    lib.gw_probe_fp64_fma_rate.argtypes = [ci, P(dbl), P(dbl), vp]
+    lib.gw_probe_fp64_fma_rate.argtypes = [ci, ci, P(dbl), P(dbl), vp]
     lib.gw_strerror.argtypes = [ci]
     lib.gw_strerror.restype = ctypes.c_char_p
     lib.gw_last_cuda_error.argtypes = [vp]
@@ -280,11 +280,11 @@ class GwContext:
         return out
 
 
-def probe_fp64_fma_rate(n_iter: int = 4096, stream=None):
-    """(fp64 FMA/s, elapsed ms) of the register-resident dependent-FMA probe kernel."""
+def probe_fp64_fma_rate(n_iter: int = 4096, mode: int = 0, stream=None):
+    """(fp64 FMA/s, elapsed ms) of the register-resident probe kernel; mode: see gw_probe_fp64_fma_rate."""
     lib = load_library()
     rate, ms = ctypes.c_double(), ctypes.c_double()
-    _check(lib.gw_probe_fp64_fma_rate(int(n_iter), ctypes.byref(rate), ctypes.byref(ms), _stream_ptr(stream)),
+    _check(lib.gw_probe_fp64_fma_rate(int(n_iter), int(mode), ctypes.byref(rate), ctypes.byref(ms), _stream_ptr(stream)),
            "gw_probe_fp64_fma_rate")
     return rate.value, ms.value
 

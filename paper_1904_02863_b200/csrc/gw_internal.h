@@ -92,6 +92,6 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
 cudaError_t configure_kernels(int *fused_ctas_per_sm);      // smem attributes + occupancy query (per n_det below)
 int         fused_ctas_per_sm(int n_det);
 size_t      fused_smem_bytes(int n_det);
-cudaError_t probe_fma_rate(int n_iter, double *fma_per_s, double *elapsed_ms, cudaStream_t s);
+cudaError_t probe_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, cudaStream_t s);
 
 } // namespace gw

@@ -657,46 +657,77 @@ cudaError_t configure_kernels(int *out)
 int fused_ctas_per_sm(int n_det) { return (n_det >= 1 && n_det <= GW_MAX_DET) ? g_ctas_per_sm[n_det] : 0; }
 
 // =====================================================================================================
-// fp64 FMA-rate probe: 8 independent dependent-FMA chains per thread, register resident.
+// fp64 rate probe: 8 independent register-resident chains per thread, 64 warps per SM.
+//   mode 0: v = fma(v, imm, imm)          one register operand            -> the pipe's peak
+//   mode 1: v = fma(a_i, b_i, v)          three distinct register operands (what a dot product needs)
+//   mode 2: v = fma(a_i, m, v)            three register operands, one shared by consecutive instructions
+//   mode 3: mma.sync m8n8k4 f64 (DMMA)    256 FMA per warp instruction
+// Measured on B200 (profiles/r1_fp64_operand_probe.md): modes 0/2/3 reach ~18.5e12 FMA/s, mode 1 only 2/3 of
+// it: a DFMA that reads three distinct 64-bit registers occupies the pipe for 3 cycles instead of 2, and DMMA
+// shares the same pipe.  This is the roofline the fused kernel is read against.
 // =====================================================================================================
-__global__ void __launch_bounds__(256) fma_probe_kernel(int n_iter, double seed, double *sink)
+template <int MODE>
+__global__ void __launch_bounds__(256) fma_probe_kernel(int n_iter, const double *in, double *sink)
 {
-    double v0 = seed + threadIdx.x, v1 = v0 + 1, v2 = v0 + 2, v3 = v0 + 3, v4 = v0 + 4, v5 = v0 + 5, v6 = v0 + 6,
-           v7 = v0 + 7;
-    const double m = 0.999999, c = 1e-9;
-    for (int i = 0; i < n_iter; ++i) {
+    double v[8], a[8], b[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        v[i] = in[threadIdx.x + i]; a[i] = in[64 + threadIdx.x + 3 * i]; b[i] = in[128 + threadIdx.x + 5 * i];
+    }
+    const double m = in[7];
+    for (int it = 0; it < n_iter; ++it) {
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            v0 = __fma_rn(v0, m, c); v1 = __fma_rn(v1, m, c); v2 = __fma_rn(v2, m, c); v3 = __fma_rn(v3, m, c);
-            v4 = __fma_rn(v4, m, c); v5 = __fma_rn(v5, m, c); v6 = __fma_rn(v6, m, c); v7 = __fma_rn(v7, m, c);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if (MODE == 0) v[i] = __fma_rn(v[i], 0.999999, 1e-9);
+                if (MODE == 1) v[i] = __fma_rn(a[i], b[i], v[i]);
+                if (MODE == 2) v[i] = __fma_rn(a[i], m, v[i]);
+                if (MODE == 3)
+                    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                 : "+d"(v[i]), "+d"(b[i]) : "d"(a[0]), "d"(m));
+            }
         }
     }
-    const double r = ((v0 + v1) + (v2 + v3)) + ((v4 + v5) + (v6 + v7));
+    double r = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) r += v[i] + b[i];
     if (r == 123.456) sink[0] = r;                           // never true; keeps the chains alive
 }
 
-cudaError_t probe_fma_rate(int n_iter, double *fma_per_s, double *elapsed_ms, cudaStream_t s)
+cudaError_t probe_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, cudaStream_t s)
 {
     int dev = 0, sms = 0;
     cudaError_t e;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    double *sink = nullptr;
-    if ((e = cudaMalloc(&sink, sizeof(double))) != cudaSuccess) return e;
+    double *buf = nullptr;
+    if ((e = cudaMalloc(&buf, 1024 * sizeof(double))) != cudaSuccess) return e;
+    cudaMemsetAsync(buf, 0, 1024 * sizeof(double), s);
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     const int blocks = sms * 8;
-    fma_probe_kernel<<<blocks, 256, 0, s>>>(n_iter / 8 + 1, 1.0, sink);        // warm-up
+    auto launch = [&](int n) {
+        switch (mode) {
+        case 1:  fma_probe_kernel<1><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        case 2:  fma_probe_kernel<2><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        case 3:  fma_probe_kernel<3><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        default: fma_probe_kernel<0><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        }
+    };
+    launch(n_iter / 8 + 1);                                  // warm-up
     cudaEventRecord(e0, s);
-    fma_probe_kernel<<<blocks, 256, 0, s>>>(n_iter, 1.0, sink);
+    launch(n_iter);
     cudaEventRecord(e1, s);
     e = cudaEventSynchronize(e1);
     float ms = 0.f;
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
     cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(sink);
+    cudaFree(buf);
     if (e != cudaSuccess) return e;
-    const double fmas = (double)blocks * 256.0 * (double)n_iter * 64.0;
+    // per thread and iteration: 64 instructions; a DMMA instruction is 256 FMA per warp = 8 per lane
+    const double per_instr = (mode == 3) ? 8.0 : 1.0;
+    const double fmas = (double)blocks * 256.0 * (double)n_iter * 64.0 * per_instr;
     if (fma_per_s) *fma_per_s = fmas / (ms * 1e-3);
     if (elapsed_ms) *elapsed_ms = ms;
     return cudaGetLastError();
