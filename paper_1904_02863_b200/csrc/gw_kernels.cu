@@ -271,44 +271,90 @@ __device__ __forceinline__ double phase_turns(const PhaseCoef &k, double2 b01, d
 // 16 B/element store stream.
 //     h_I(f) = CA_I f^(-7/6) exp(-2 pi i (Phi'(f) + f tau_I))
 // =====================================================================================================
-constexpr int kWfProps = 8;
+constexpr int kWfProps = 8;      // proposals per CTA
+constexpr int kWfBins  = 2;      // bins per thread (kThreads * kWfBins bins per CTA)
 
 struct WaveArgs {
     const double *planes, *fm76, *freq, *rec;
     int64_t n_pad, n_bins, n_prop, rec_stride;
-    int     n_det, bin_blocks;
+    int     bin_blocks;
     double *h;
 };
 
+template <int NDET>
 __global__ void __launch_bounds__(kThreads) waveform_kernel(const WaveArgs a)
 {
+    constexpr int NF = 10 + 4 * NDET;            // doubles per staged record: 9 coefs + pad, (tau, pad, CAre, CAim) per det
+    __shared__ __align__(16) double srec[kWfProps][NF];
+    const int     tid     = threadIdx.x;
     const int     bin_blk = blockIdx.x % a.bin_blocks;
     const int64_t p_blk   = blockIdx.x / a.bin_blocks;
-    const int64_t j       = (int64_t)bin_blk * kThreads + threadIdx.x;
-    const bool    in      = j < a.n_bins;
-    const int64_t jc      = in ? j : a.n_bins - 1;
     const double2 *pl = reinterpret_cast<const double2 *>(a.planes);
-    const double2 b01 = pl[0 * a.n_pad + jc], b23 = pl[1 * a.n_pad + jc];
-    const double2 b45 = pl[2 * a.n_pad + jc], b67 = pl[3 * a.n_pad + jc];
-    const double  amp = a.fm76[jc], f = a.freq[jc];
-    pdl_wait_primary();
+    double2 b01[kWfBins], b23[kWfBins], b45[kWfBins], b67[kWfBins];
+    double  amp[kWfBins], f[kWfBins];
+    int64_t j[kWfBins];
+    bool    in[kWfBins];
+#pragma unroll
+    for (int u = 0; u < kWfBins; ++u) {
+        j[u]  = ((int64_t)bin_blk * kWfBins + u) * kThreads + tid;
+        in[u] = j[u] < a.n_bins;
+        const int64_t jc = in[u] ? j[u] : a.n_bins - 1;
+        b01[u] = pl[0 * a.n_pad + jc]; b23[u] = pl[1 * a.n_pad + jc];
+        b45[u] = pl[2 * a.n_pad + jc]; b67[u] = pl[3 * a.n_pad + jc];
+        amp[u] = a.fm76[jc]; f[u] = a.freq[jc];
+    }
+    pdl_wait_primary();                          // the records come from the setup kernel
     const int64_t b0 = p_blk * kWfProps;
-    const int64_t b1 = (b0 + kWfProps < a.n_prop) ? b0 + kWfProps : a.n_prop;
+    const int     np = (int)((b0 + kWfProps < a.n_prop) ? kWfProps : a.n_prop - b0);
+    for (int idx = tid; idx < np * NF; idx += kThreads) {
+        const int p = idx / NF, fld = idx % NF;
+        double v = 0.0;
+        if (fld < 9) v = a.rec[(int64_t)fld * a.rec_stride + b0 + p];
+        else if (fld >= 10) {
+            const int i = (fld - 10) >> 2, w = (fld - 10) & 3;          // w: 0 tau, 2 CAre, 3 CAim
+            if (w != 1) v = a.rec[(int64_t)(9 + kRecPerDet * i + (w == 0 ? 0 : w - 1)) * a.rec_stride + b0 + p];
+        }
+        srec[p][fld] = v;
+    }
+    __syncthreads();
     double2 *h = reinterpret_cast<double2 *>(a.h);
-    for (int64_t b = b0; b < b1; ++b) {
-        const PhaseCoef k = load_coef(a.rec, a.rec_stride, b);       // warp-uniform loads
-        const double ph = phase_turns(k, b01, b23, b45, b67);
-        for (int i = 0; i < a.n_det; ++i) {
-            const double *ri = a.rec + (int64_t)(9 + kRecPerDet * i) * a.rec_stride + b;
-            const double tau = ri[0], car = ri[a.rec_stride], cai = ri[2 * a.rec_stride];
-            double c, s;
-            cis_turns(__fma_rn(f, tau, ph), c, s);
-            const double kr = car * amp, ki = cai * amp;
-            // (kr + i ki)(c - i s)
-            const double2 out = make_double2(__fma_rn(kr, c, ki * s), __fma_rn(ki, c, -(kr * s)));
-            if (in) __stcs(&h[(b * a.n_det + i) * a.n_bins + j], out);
+    for (int p = 0; p < np; ++p) {
+        const double2 *r2 = reinterpret_cast<const double2 *>(srec[p]);  // warp-broadcast LDS.128
+        const double2 k01 = r2[0], k23 = r2[1], k45 = r2[2], k67 = r2[3], k8 = r2[4];
+        PhaseCoef k;
+        k.c0 = k01.x; k.c2 = k01.y; k.c3 = k23.x; k.c4 = k23.y; k.c5 = k45.x; k.cL5 = k45.y;
+        k.c6 = k67.x; k.cL6 = k67.y; k.c7 = k8.x;
+        double ph[kWfBins];
+#pragma unroll
+        for (int u = 0; u < kWfBins; ++u) ph[u] = phase_turns(k, b01[u], b23[u], b45[u], b67[u]);
+        double2 *row = h + ((b0 + p) * NDET) * a.n_bins;
+#pragma unroll
+        for (int i = 0; i < NDET; ++i) {
+            const double2 t_ = r2[5 + 2 * i], ca = r2[6 + 2 * i];      // (tau, -), (CAre, CAim)
+#pragma unroll
+            for (int u = 0; u < kWfBins; ++u) {
+                double c, s;
+                cis_turns(__fma_rn(f[u], t_.x, ph[u]), c, s);
+                const double kr = ca.x * amp[u], ki = ca.y * amp[u];
+                // (kr + i ki)(c - i s)
+                const double2 out = make_double2(__fma_rn(kr, c, ki * s), __fma_rn(ki, c, -(kr * s)));
+                if (in[u]) __stcs(row + j[u], out);
+            }
+            row += a.n_bins;
         }
     }
+}
+
+template <int NDET>
+static cudaError_t launch_waveform_t(const WaveArgs &a, int64_t blocks, cudaStream_t s)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, waveform_kernel<NDET>, a);
 }
 
 cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, int64_t rec_stride,
@@ -317,19 +363,19 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
     WaveArgs a;
     a.planes = t.planes; a.fm76 = t.fm76; a.freq = t.freq; a.rec = rec;
     a.n_pad = t.n_pad; a.n_bins = t.n_bins; a.n_prop = n_prop; a.rec_stride = rec_stride;
-    a.n_det = t.n_det; a.bin_blocks = (int)((t.n_bins + kThreads - 1) / kThreads);
+    a.bin_blocks = (int)((t.n_bins + kThreads * kWfBins - 1) / (kThreads * kWfBins));
     a.h = h_out;
     const int64_t p_blocks = (n_prop + kWfProps - 1) / kWfProps;
     const int64_t blocks = p_blocks * a.bin_blocks;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)blocks); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = 0; cfg.stream = s;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
     *launches += 1;
-    return cudaLaunchKernelEx(&cfg, waveform_kernel, a);
+    switch (t.n_det) {
+    case 1: return launch_waveform_t<1>(a, blocks, s);
+    case 2: return launch_waveform_t<2>(a, blocks, s);
+    case 3: return launch_waveform_t<3>(a, blocks, s);
+    case 4: return launch_waveform_t<4>(a, blocks, s);
+    default: return cudaErrorInvalidValue;
+    }
 }
 
 // =====================================================================================================
