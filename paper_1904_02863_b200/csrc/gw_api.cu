@@ -263,8 +263,6 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
         ctx->ctas_per_sm = fused_ctas_per_sm(n_det);
         bool ok = true;
         ok = ok && (e = cudaMalloc(&t.planes, sizeof(double) * 2 * (kBasisPlanes + n_det) * t.n_pad)) == cudaSuccess;
-        ok = ok && (e = cudaMalloc(&t.fm76, sizeof(double) * t.n_pad)) == cudaSuccess;
-        ok = ok && (e = cudaMalloc(&t.freq, sizeof(double) * t.n_pad)) == cudaSuccess;
         ok = ok && (e = cudaMalloc(&dfreq, sizeof(double) * nf)) == cudaSuccess;
         ok = ok && (e = cudaMalloc(&ddata, sizeof(double) * nd * 2)) == cudaSuccess;
         ok = ok && (e = cudaMalloc(&dpsd, sizeof(double) * nd)) == cudaSuccess;
@@ -300,7 +298,7 @@ int gw_ctx_destroy(gw_ctx *ctx)
     if (!ctx) return GW_OK;
     cudaDeviceSynchronize();
     free_workspace(ctx->w);
-    cudaFree(ctx->t.planes); cudaFree(ctx->t.fm76); cudaFree(ctx->t.freq);
+    cudaFree(ctx->t.planes);
     for (int i = 0; i < 3; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
     cudaGetLastError();
@@ -374,7 +372,7 @@ int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *l
     if (partial_need(ctx, p) > ctx->w.partial_doubles || p.n_tiles > ctx->w.n_tickets) return GW_ERR_INVALID_ARG;
     if (ctx->timing) cudaEventRecord(ctx->ev[0], s);
     cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
-                                 ctx->w.rec_stride, (double)p.lpp * ctx->t.delta_f, s, &ctx->launches);
+                                 ctx->w.rec_stride, (double)p.lpp * ctx->t.delta_f, 1, s, &ctx->launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     if (ctx->timing) cudaEventRecord(ctx->ev[1], s);
     e = launch_fused(ctx->t, p, n_prop, ctx->w.rec, ctx->w.rec_stride, ctx->w.partial, ctx->w.tickets, lnl_out_dev,
@@ -392,7 +390,7 @@ int gw_waveform_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, doub
     cudaStream_t s = (cudaStream_t)cuda_stream;
     if (ctx->timing) cudaEventRecord(ctx->ev[0], s);
     cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
-                                 ctx->w.rec_stride, ctx->t.delta_f, s, &ctx->launches);
+                                 ctx->w.rec_stride, ctx->t.delta_f, 0, s, &ctx->launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     if (ctx->timing) cudaEventRecord(ctx->ev[1], s);
     e = launch_waveform(ctx->t, n_prop, ctx->w.rec, ctx->w.rec_stride, h_out_dev, s, &ctx->launches);

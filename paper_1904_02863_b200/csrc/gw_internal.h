@@ -30,7 +30,7 @@ constexpr int kStageBins  = GW_STAGE_BINS;  // bins per shared-memory stage of t
 constexpr int kStages     = GW_STAGES;      // stage ring depth
 constexpr int kUnroll     = GW_UNROLL;      // bins per unrolled trip of the fused hot loop
 constexpr int kBasis      = 8;     // per-bin phase basis values (4 planes of 2)
-constexpr int kBasisPlanes = 4;
+constexpr int kBasisPlanes = 5;    // (x^-5,x^-3) (x^-2,x^-1) (ln f,x) (x ln f,x^2) (f,f^-7/6)
 constexpr int kRecFixed   = 10;    // record fields before the per-detector block
 constexpr int kRecPerDet  = 5;     // tau, Cre, Cim, rot_re, rot_im
 
@@ -49,9 +49,7 @@ struct Tables {
     int64_t n_pad;        // allocated bins per plane (>= M, multiple of 32)
     int     n_det;
     double  f0, delta_f;
-    double *planes;       // [4 + n_det][n_pad][2]: basis planes (x^-5,x^-3) (x^-2,x^-1) (ln f,x) (x ln f,x^2), then g_I (re,im)
-    double *fm76;         // [n_pad]  f^(-7/6)
-    double *freq;         // [n_pad]  f_j
+    double *planes;       // [5 + n_det][n_pad][2]: the five basis planes above, then g_I (re,im) per detector
     double  i7[GW_MAX_DET];   // host copy of I7_I = sum_j (4 df/S_Ij) f_j^(-7/3)
 };
 
@@ -83,7 +81,7 @@ cudaError_t launch_precompute(const Tables &t, const double *freqs_dev, const do
                               const double *psd_dev, double *i7_dev, cudaStream_t s, int64_t *launches);
 cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int spin_order, int64_t n_prop,
                          const double *theta_dev, double *rec, int64_t rec_stride, double rot_stride_hz,
-                         cudaStream_t s, int64_t *launches);
+                         int relative_tau, cudaStream_t s, int64_t *launches);
 cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, const double *rec,
                          int64_t rec_stride, double *partial, unsigned int *tickets, double *lnl_out,
                          double *parts_out, cudaStream_t s, int64_t *launches);

@@ -24,8 +24,7 @@ namespace gw {
 // =====================================================================================================
 __global__ void precompute_kernel(int64_t n_bins, int64_t n_pad, int n_det, double f0, double delta_f,
                                   const double *__restrict__ freqs, const double *__restrict__ data_ri,
-                                  const double *__restrict__ psd, double *__restrict__ planes,
-                                  double *__restrict__ fm76, double *__restrict__ freq)
+                                  const double *__restrict__ psd, double *__restrict__ planes)
 {
     const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n_pad) return;
@@ -42,8 +41,7 @@ __global__ void precompute_kernel(int64_t n_bins, int64_t n_pad, int n_det, doub
         pl[2 * n_pad + j] = make_double2(L, x);              // ln f, x
         pl[3 * n_pad + j] = make_double2(x * L, x * x);      // x ln f, x^2
         const double a = 1.0 / (f * sqrt(x));                // f^(-7/6)
-        fm76[j] = a;
-        freq[j] = f;
+        pl[4 * n_pad + j] = make_double2(f, a);              // f, f^(-7/6)
         for (int i = 0; i < n_det; ++i) {
             const double w  = 4.0 * delta_f / psd[(int64_t)i * n_bins + j];
             const double wa = w * a;
@@ -55,8 +53,7 @@ __global__ void precompute_kernel(int64_t n_bins, int64_t n_pad, int n_det, doub
         pl[1 * n_pad + j] = make_double2(1.0, 1.0);
         pl[2 * n_pad + j] = make_double2(0.0, 1.0);
         pl[3 * n_pad + j] = make_double2(0.0, 1.0);
-        fm76[j] = 0.0;
-        freq[j] = f0 + (double)j * delta_f;
+        pl[4 * n_pad + j] = make_double2(f0 + (double)j * delta_f, 0.0);
         for (int i = 0; i < n_det; ++i) pl[(int64_t)(kBasisPlanes + i) * n_pad + j] = make_double2(0.0, 0.0);
     }
 }
@@ -65,13 +62,13 @@ __global__ void precompute_kernel(int64_t n_bins, int64_t n_pad, int n_det, doub
 // strided slice, then a fixed shared-memory tree (deterministic).
 __global__ void __launch_bounds__(1024) norm_kernel(int64_t n_bins, double delta_f,
                                                     const double *__restrict__ psd,
-                                                    const double *__restrict__ fm76, double *__restrict__ i7)
+                                                    const double2 *__restrict__ f_amp, double *__restrict__ i7)
 {
     __shared__ double sh[1024];
     const int i = blockIdx.x;
     double s = 0.0, c = 0.0;
     for (int64_t j = threadIdx.x; j < n_bins; j += 1024) {
-        const double a = fm76[j];
+        const double a = f_amp[j].y;                          // f^(-7/6)
         const double v = (4.0 * delta_f / psd[(int64_t)i * n_bins + j]) * (a * a);
         const double t = s + v;                               // terms are positive: |s| >= |v| after the first
         c += (fabs(s) >= fabs(v)) ? ((s - t) + v) : ((v - t) + s);
@@ -92,10 +89,11 @@ cudaError_t launch_precompute(const Tables &t, const double *freqs_dev, const do
     const int threads = 256;
     const unsigned blocks = (unsigned)((t.n_pad + threads - 1) / threads);
     precompute_kernel<<<blocks, threads, 0, s>>>(t.n_bins, t.n_pad, t.n_det, t.f0, t.delta_f, freqs_dev,
-                                                 data_dev, psd_dev, t.planes, t.fm76, t.freq);
+                                                 data_dev, psd_dev, t.planes);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    norm_kernel<<<t.n_det, 1024, 0, s>>>(t.n_bins, t.delta_f, psd_dev, t.fm76, i7_dev);
+    norm_kernel<<<t.n_det, 1024, 0, s>>>(t.n_bins, t.delta_f, psd_dev,
+                                         reinterpret_cast<const double2 *>(t.planes) + 4 * t.n_pad, i7_dev);
     *launches += 2;
     return cudaGetLastError();
 }
@@ -116,6 +114,7 @@ struct SetupArgs {
     const double *theta;
     double *rec;
     double  rot_stride_hz;
+    int     relative_tau;     // 1: tau_I (I >= 1) and rot_I are relative to detector 0 (fused kernel); 0: absolute
 };
 
 __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
@@ -194,6 +193,7 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
     const double n[3] = {cd * cg, -cd * sg, sd};             // cos(ra - gmst) = cg, sin(ra - gmst) = -sg
     const double pol_plus = 0.5 * (1.0 + cosi * cosi);
 
+    double tau0 = 0.0;
     for (int i = 0; i < a.n_det; ++i) {
         const DetGeom &g = a.dets.d[i];
         double fp, fc, dt;
@@ -211,7 +211,9 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
             fc = 2.0 * (X[0] * DY[0] + X[1] * DY[1] + X[2] * DY[2]);
             dt = -(g.rc[0] * n[0] + g.rc[1] * n[1] + g.rc[2] * n[2]);
         }
-        const double tau = tc + dt;
+        double tau = tc + dt;
+        if (i == 0) tau0 = tau;
+        else if (a.relative_tau) tau -= tau0;
         double rc_, rs_;
         cis_turns_of_product(-a.rot_stride_hz, tau, rc_, rs_);
         double *ri = r + (int64_t)(9 + kRecPerDet * i) * S;
@@ -225,12 +227,12 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
 
 cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int spin_order, int64_t n_prop,
                          const double *theta_dev, double *rec, int64_t rec_stride, double rot_stride_hz,
-                         cudaStream_t s, int64_t *launches)
+                         int relative_tau, cudaStream_t s, int64_t *launches)
 {
     SetupArgs a;
     a.dets = dets; a.gmst = gmst; a.n_det = t.n_det; a.spin_order = spin_order;
     a.n_prop = n_prop; a.rec_stride = rec_stride; a.theta = theta_dev; a.rec = rec;
-    a.rot_stride_hz = rot_stride_hz;
+    a.rot_stride_hz = rot_stride_hz; a.relative_tau = relative_tau;
     const unsigned blocks = (unsigned)((n_prop + 127) / 128);
     setup_kernel<<<blocks, 128, 0, s>>>(a);
     *launches += 1;
@@ -275,7 +277,7 @@ constexpr int kWfProps = 8;      // proposals per CTA
 constexpr int kWfBins  = 2;      // bins per thread (kThreads * kWfBins bins per CTA)
 
 struct WaveArgs {
-    const double *planes, *fm76, *freq, *rec;
+    const double *planes, *rec;
     int64_t n_pad, n_bins, n_prop, rec_stride;
     int     bin_blocks;
     double *h;
@@ -301,7 +303,8 @@ __global__ void __launch_bounds__(kThreads) waveform_kernel(const WaveArgs a)
         const int64_t jc = in[u] ? j[u] : a.n_bins - 1;
         b01[u] = pl[0 * a.n_pad + jc]; b23[u] = pl[1 * a.n_pad + jc];
         b45[u] = pl[2 * a.n_pad + jc]; b67[u] = pl[3 * a.n_pad + jc];
-        amp[u] = a.fm76[jc]; f[u] = a.freq[jc];
+        const double2 fa = pl[4 * a.n_pad + jc];
+        f[u] = fa.x; amp[u] = fa.y;
     }
     pdl_wait_primary();                          // the records come from the setup kernel
     const int64_t b0 = p_blk * kWfProps;
@@ -361,7 +364,7 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
                             double *h_out, cudaStream_t s, int64_t *launches)
 {
     WaveArgs a;
-    a.planes = t.planes; a.fm76 = t.fm76; a.freq = t.freq; a.rec = rec;
+    a.planes = t.planes; a.rec = rec;
     a.n_pad = t.n_pad; a.n_bins = t.n_bins; a.n_prop = n_prop; a.rec_stride = rec_stride;
     a.bin_blocks = (int)((t.n_bins + kThreads * kWfBins - 1) / (kThreads * kWfBins));
     a.h = h_out;
@@ -524,6 +527,10 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                     for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.cL6, v[u].x, ph[u]);
 #pragma unroll
                     for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.c7, v[u].y, ph[u]);
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) v[u] = P[4 * kStageBins + it + u];
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(tau[0], v[u].x, ph[u]);   // + f tau_0
                 }
 #pragma unroll
                 for (int u = 0; u < kUnroll; ++u) cis_turns(ph[u], cs[u], sn[u]);
@@ -532,6 +539,11 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
 #pragma unroll
                     for (int i = 0; i < NDET; ++i) {
                         const double2 g = P[(kBasisPlanes + i) * kStageBins + it + u];
+                        if (i == 0) {                                         // reference detector: no rotation
+                            zr[0] = __fma_rn(-g.y, sn[u], __fma_rn(g.x, cs[u], zr[0]));
+                            zi[0] = __fma_rn(g.y, cs[u], __fma_rn(g.x, sn[u], zi[0]));
+                            continue;
+                        }
                         const double t1 = g.y * sn[u];
                         const double t2 = g.y * cs[u];
                         const double a2 = __fma_rn(g.x, cs[u], -t1);          // Re g e^{+i 2 pi Phi'}
@@ -549,14 +561,20 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             int jj = MULTI ? sub + it * lpp : it;
             bool masked = false;
             if (MULTI) { masked = jj >= cnt; jj = masked ? cnt - 1 : jj; }
-            const double ph = phase_turns(k, P[0 * kStageBins + jj], P[1 * kStageBins + jj],
-                                          P[2 * kStageBins + jj], P[3 * kStageBins + jj]);
+            double ph = phase_turns(k, P[0 * kStageBins + jj], P[1 * kStageBins + jj],
+                                    P[2 * kStageBins + jj], P[3 * kStageBins + jj]);
+            ph = __fma_rn(tau[0], P[4 * kStageBins + jj].x, ph);
             double c, sn;
             cis_turns(ph, c, sn);
 #pragma unroll
             for (int i = 0; i < NDET; ++i) {
                 double2 g = P[(kBasisPlanes + i) * kStageBins + jj];
                 if (MULTI && masked) g = make_double2(0.0, 0.0);
+                if (i == 0) {
+                    zr[0] = __fma_rn(-g.y, sn, __fma_rn(g.x, c, zr[0]));
+                    zi[0] = __fma_rn(g.y, c, __fma_rn(g.x, sn, zi[0]));
+                    continue;
+                }
                 const double wr = __fma_rn(g.x, c, -(g.y * sn));     // g * e^{+i 2 pi Phi'}
                 const double wi = __fma_rn(g.x, sn, g.y * c);
                 const double nr = __fma_rn(zr[i], rr[i], __fma_rn(-zi[i], ri_[i], wr));
@@ -569,12 +587,13 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
         if (tid == 0 && s + kStages < n_stage) issue_stage(s + kStages);
     }
 
-    // seed: multiply by exp(+2 pi i f_last tau_I), f_last = frequency of this thread's last iteration
+    // seed (detectors >= 1): multiply by exp(+2 pi i f_last (tau_I - tau_0)), f_last = frequency of this
+    // thread's last iteration
     {
         const int64_t j_last = j0 + sub + (int64_t)(iters_total - 1) * lpp;
         const double f_last = __fma_rn((double)j_last, a.delta_f, a.f0);
 #pragma unroll
-        for (int i = 0; i < NDET; ++i) {
+        for (int i = 1; i < NDET; ++i) {
             double c, sn;
             cis_turns_of_product(f_last, tau[i], c, sn);
             const double nr = __fma_rn(zr[i], c, -(zi[i] * sn));
