@@ -34,6 +34,9 @@ METRIC = "likelihood evals/sec (fp64, waveform+lnL)"
 UNIT = "lnL/s"
 FP64_LANES_PER_SM = 64          # B200 fp64 FMA lanes per SM (37.2 TFLOP/s at 1965 MHz x 148 SMs)
 L2_FLUSH_BYTES = 256 << 20
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/*_fused_ncu_summary.md); None where no capture exists for the workload.
+NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 1.72e6}
 
 
 def parse_workload(spec):
@@ -114,18 +117,22 @@ def build_problem(cfg, batch_total):
 
 
 def oracle_rate(cfg, f, S, dets, d, th, target_s, n_threads=0):
-    """Time the oracle, as it stands, on a bounded prefix of the proposals (~target_s of CPU work)."""
+    """Time the oracle, as it stands, for about target_s seconds of wall time on a bounded sample of the
+    workload: a prefix of the proposals, passed over repeatedly if the whole batch is quicker than target_s."""
     import oracle
     oracle.build()
-    pilot = th[: min(len(th), max(2, os.cpu_count() or 1))]
+    pilot = th[: min(len(th), max(2, 2 * (os.cpu_count() or 1)))]
+    oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, pilot, cfg.spin_order, n_threads)      # thread start-up
     t0 = time.perf_counter()
-    _, _, used = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, pilot, cfg.spin_order, n_threads)
+    oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, pilot, cfg.spin_order, n_threads)
     dt = max(time.perf_counter() - t0, 1e-6)
     n = int(min(len(th), max(len(pilot), len(pilot) * target_s / dt)))
+    passes = max(1, int(round(target_s / max(dt * n / len(pilot), 1e-6))))
     t0 = time.perf_counter()
-    _, _, used = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order, n_threads)
+    for _ in range(passes):
+        _, _, used = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order, n_threads)
     dt = time.perf_counter() - t0
-    return n / dt, used, n, dt
+    return n * passes / dt, used, n, dt, passes
 
 
 def run_reference(args):
@@ -142,7 +149,7 @@ def run_reference(args):
     th = inputs.proposals(cfg)[:batch] if batch <= cfg.batch else inputs.proposals(cfg)
     # size one step to ~ (90 s budget) / (steps + warmup)
     per_step_s = min(10.0, 90.0 / max(1, args.steps + args.warmup))
-    rate, used, n, _ = oracle_rate(cfg, f, S, dets, d, th, per_step_s)
+    rate, used, n, _, _ = oracle_rate(cfg, f, S, dets, d, th, min(per_step_s, 3.0))
     n = max(1, min(len(th), int(rate * per_step_s)))
     for _ in range(args.warmup):
         oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order)
@@ -255,7 +262,7 @@ def run_ours(args):
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     peak = n_sm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     roofline = {"bound": "alu", "kernel": "fused_kernel<%d>" % n_det, "achieved": achieved, "peak": peak,
-                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(name) if B == cfg.batch else None,
                 "peak_source": "derived: %d SMs x %d fp64 FMA lanes x 2 flop x %.0f MHz (MEASURED_PEAKS sm_max_mhz)"
                                % (n_sm, FP64_LANES_PER_SM, sm_max),
                 "peak_measured_fma_probe": 2 * fma_rate / 1e12, "frac_of_measured": achieved / (2 * fma_rate / 1e12),
@@ -308,9 +315,9 @@ def run_ours(args):
     # ---- CPU baseline: the oracle as it stands on this box's host cores (rank 0, N = 1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        rate, used, n, dt = oracle_rate(cfg, f, S, dets, d, th, args.cpu_seconds)
+        rate, used, n, dt, passes = oracle_rate(cfg, f, S, dets, d, th, args.cpu_seconds)
         cpu = {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle",
-               "sample": f"first {n} of {B} proposals, all {M} bins x {n_det} detectors, {dt:.1f} s"}
+               "sample": f"first {n} of {B} proposals x {passes} passes, all {M} bins x {n_det} detectors, {dt:.1f} s wall"}
 
     clocks = clk.summary()
     ctx.close()
@@ -333,7 +340,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C1")

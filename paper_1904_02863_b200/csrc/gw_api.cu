@@ -52,6 +52,8 @@ constexpr double kProBins  = 14.0;
 constexpr double kSatWarps = 3.0;
 constexpr int    kMaxChunks = 4096;
 constexpr int64_t kMaxWaves = 8;
+constexpr double kMultiPenalty = 1.35;     // the lanes-interleaved loop costs this much more per bin (measured, C2)
+constexpr double kFinishPerChunk = 0.25;   // last-CTA cross-chunk sum, in bin-sweep equivalents per chunk
 
 Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
 {
@@ -72,13 +74,14 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
         for (int64_t nc = 1; nc <= max_chunks; ++nc) {
             const int64_t ctas = tiles * nc;
             const int64_t chunk = (M + nc - 1) / nc;
-            const double per_thread = (double)((chunk + lpp - 1) / lpp) + kProBins + (lpp > 1 ? 2.0 : 0.0);
+            const double per_thread = (double)((chunk + lpp - 1) / lpp) * (lpp > 1 ? kMultiPenalty : 1.0) + kProBins +
+                                      (lpp > 1 ? 2.0 : 0.0);
             const int64_t per_sm = (ctas + n_sm - 1) / n_sm;                  // CTAs an SM must run
             const int64_t waves = (per_sm + slots_per_sm - 1) / slots_per_sm;
             const double resident = (double)per_sm / (double)waves;           // average co-resident CTAs
             const double warps_per_sched = resident * (kThreads / 32) / 4.0;
             const double slowdown = warps_per_sched > kSatWarps ? warps_per_sched / kSatWarps : 1.0;
-            const double cost = (double)waves * per_thread * slowdown + 1e-3 * (double)nc;
+            const double cost = (double)waves * per_thread * slowdown + kFinishPerChunk * (double)nc;
             if (cost < best_cost) {
                 best_cost = cost;
                 best.lpp = lpp; best.props_per_cta = pt; best.n_chunks = (int)nc; best.n_tiles = tiles;

@@ -638,7 +638,23 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
 #pragma unroll
             for (int i = 0; i < NDET; ++i) { sr[i] = 0.0; si[i] = 0.0; }
             const double *base = a.partial + (tile * a.n_chunks * (int64_t)(2 * NDET)) * PT + tid;
-            for (int c = 0; c < a.n_chunks; ++c) {
+            // loads of kFinishBatch chunks are issued together (the sum is latency-bound on L2 otherwise);
+            // the additions stay in chunk-index order, so the result does not depend on the batching.
+            constexpr int kFinishBatch = 8;
+            int c = 0;
+            for (; c + kFinishBatch <= a.n_chunks; c += kFinishBatch) {
+                double v[kFinishBatch][2 * NDET];
+#pragma unroll
+                for (int u = 0; u < kFinishBatch; ++u)
+#pragma unroll
+                    for (int q = 0; q < 2 * NDET; ++q)
+                        v[u][q] = __ldcg(base + ((int64_t)(c + u) * 2 * NDET + q) * PT);
+#pragma unroll
+                for (int u = 0; u < kFinishBatch; ++u)
+#pragma unroll
+                    for (int i = 0; i < NDET; ++i) { sr[i] += v[u][2 * i]; si[i] += v[u][2 * i + 1]; }
+            }
+            for (; c < a.n_chunks; ++c) {
 #pragma unroll
                 for (int i = 0; i < NDET; ++i) {
                     sr[i] += __ldcg(base + ((int64_t)c * 2 * NDET + 2 * i) * PT);
