@@ -99,7 +99,7 @@ cudaError_t launch_precompute(const Tables &t, const double *freqs_dev, const do
 }
 
 // =====================================================================================================
-// K1: per-proposal setup (step a1).  One thread per proposal; record fields are stored SoA
+// K1: per-proposal setup (step a1).  Four warps share 32 proposals by role; record fields are stored SoA
 // (rec[field * rec_stride + b]) so that the thread-per-proposal kernels read them coalesced.
 //   fields 0..8 : c0 c2 c3 c4 c5 cL5 c6 cL6 c7    (phase coefficients in turns, see file header)
 //   per detector I (base 9 + 5 I): tau_I = t_c + dt_I ; CA_I = A0 * C_I (re, im) ;
@@ -117,73 +117,87 @@ struct SetupArgs {
     int     relative_tau;     // 1: tau_I (I >= 1) and rot_I are relative to detector 0 (fused kernel); 0: absolute
 };
 
+// A CTA of 128 threads serves 32 proposals; warp w takes role w for proposal (block*32 + lane), so the four
+// parts of the record are computed concurrently and no warp diverges:
+//   role 0: masses and the nine phase coefficients (O1-O3)
+//   role 1..3: amplitude, sky frame and the detector block(s) (O4-O6): role r takes detector r-1, and role 3
+//              also detector 3 when n_det = 4.  Each detector role recomputes the (cheap) amplitude and frame.
 __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
 {
     pdl_launch_dependents();          // the dependent kernel may start its table prefetch now
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int role = threadIdx.x >> 5;
+    const int64_t b = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
     if (b >= a.n_prop) return;
     const double *th = a.theta + b * GW_NPARAM;
-    const double mc = th[GW_P_MC], q = th[GW_P_Q], chi1 = th[GW_P_CHI1], chi2 = th[GW_P_CHI2];
+    double *r = a.rec + b;
+    const int64_t S = a.rec_stride;
+    const double mc = th[GW_P_MC];
+
+    if (role == 0) {
+        const double q = th[GW_P_Q], chi1 = th[GW_P_CHI1], chi2 = th[GW_P_CHI2], phic = th[GW_P_PHIC];
+        // O1: masses.  kappa = (pi M)^(1/3) = (pi Mc)^(1/3) eta^(-1/5)
+        const double opq   = 1.0 + q;
+        const double eta   = q / (opq * opq);
+        const double delta = (1.0 - q) / opq;                    // mu1 - mu2
+        const double kc    = cbrt(kPi * mc * kTsun);             // (pi Mc)^(1/3): the 0PN term depends on Mc only
+        const double ln_eta = log(eta);
+        const double kap   = kc * exp(-0.2 * ln_eta);
+        const double lnk   = log(kc) - 0.2 * ln_eta;
+        const double ikap  = 1.0 / kap;
+        // O2: phase coefficients; spin terms in the chi_s / chi_a coding
+        double four_beta = 0.0, m10_sigma = 0.0;
+        if (a.spin_order >= 1) {
+            const double xs = 0.5 * (chi1 + chi2), xa = 0.5 * (chi1 - chi2);
+            four_beta = (113.0 / 3.0 - 76.0 / 3.0 * eta) * xs + 113.0 / 3.0 * delta * xa;
+            m10_sigma = (-405.0 / 8.0 + 2.5 * eta) * xs * xs + (-405.0 / 8.0 + 200.0 * eta) * xa * xa -
+                        405.0 / 4.0 * delta * xs * xa;
+        }
+        const double eta2 = eta * eta;
+        const double phi2 = 3715.0 / 756.0 + 55.0 / 9.0 * eta;
+        const double phi3 = -16.0 * kPi + four_beta;
+        const double phi4 = 15293365.0 / 508032.0 + 27145.0 / 504.0 * eta + 3085.0 / 72.0 * eta2 + m10_sigma;
+        const double phi5 = kPi * (38645.0 / 756.0 - 65.0 / 9.0 * eta);
+        const double ph5l = 3.0 * phi5;
+        constexpr double k6const = 11583231236531.0 / 4694215680.0 - 640.0 / 3.0 * kPi * kPi -
+                                   6848.0 / 21.0 * (kEulerG + kLn4);
+        const double phi6 = k6const + eta * (-15737765635.0 / 3048192.0 + 2255.0 / 12.0 * kPi * kPi) +
+                            76055.0 / 1728.0 * eta2 - 127825.0 / 1296.0 * eta2 * eta;
+        constexpr double ph6l = -6848.0 / 21.0;
+        const double phi7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * eta2);
+        // x-form, in turns: prefactor 3/(128 eta) / (2 pi); kappa^(k-5) x^(k-5)
+        const double pref = 3.0 / (128.0 * eta) / kTwoPi;
+        const double kc2  = kc * kc;
+        const double ik2  = ikap * ikap;
+        r[0 * S] = (3.0 / 128.0 / kTwoPi) / (kc2 * kc2 * kc);                       // c0  * x^-5
+        r[1 * S] = pref * phi2 * ik2 * ikap;                                        // c2  * x^-3
+        r[2 * S] = pref * phi3 * ik2;                                               // c3  * x^-2
+        r[3 * S] = pref * phi4 * ikap;                                              // c4  * x^-1
+        r[4 * S] = pref * (phi5 + ph5l * lnk) - (phic + 0.25 * kPi) / kTwoPi;       // c5  (constant)
+        r[5 * S] = pref * ph5l / 3.0;                                               // cL5 * ln f
+        r[6 * S] = pref * kap * (phi6 + ph6l * lnk);                                // c6  * x
+        r[7 * S] = pref * kap * ph6l / 3.0;                                         // cL6 * x ln f
+        r[8 * S] = pref * kap * kap * phi7;                                         // c7  * x^2
+        return;
+    }
+
+    // ---- detector roles ----
+    const int i_first = role - 1;
+    const int i_last  = (role == 3 && a.n_det > 3) ? a.n_det - 1 : i_first;
+    if (i_first >= a.n_det) return;
+    const double q = th[GW_P_Q], chi1 = th[GW_P_CHI1], chi2 = th[GW_P_CHI2];
     const double dl = th[GW_P_DL], tc = th[GW_P_TC], phic = th[GW_P_PHIC], cosi = th[GW_P_COSI];
     const double ra = th[GW_P_RA], dec = th[GW_P_DEC], psi = th[GW_P_PSI];
-
     bool ok = (mc > 0.0) && (q > 0.0) && (q <= 1.0) && (dl > 0.0) && (fabs(cosi) <= 1.0) &&
               (fabs(chi1) <= 1.0) && (fabs(chi2) <= 1.0);
     ok = ok && isfinite(mc) && isfinite(dl) && isfinite(tc) && isfinite(phic) && isfinite(ra) &&
          isfinite(dec) && isfinite(psi);
-
-    // O1: masses
-    const double opq   = 1.0 + q;
-    const double eta   = q / (opq * opq);
-    const double delta = (1.0 - q) / opq;                    // mu1 - mu2
-    const double mtot  = mc * pow(eta, -0.6) * kTsun;        // seconds
-    const double kap   = cbrt(kPi * mtot);                   // kappa = (pi M)^(1/3)
-    const double lnk   = log(kap);
-    const double ikap  = 1.0 / kap;
-
-    // O2: phase coefficients; spin terms in the chi_s / chi_a coding
-    double four_beta = 0.0, m10_sigma = 0.0;
-    if (a.spin_order >= 1) {
-        const double xs = 0.5 * (chi1 + chi2), xa = 0.5 * (chi1 - chi2);
-        four_beta = (113.0 / 3.0 - 76.0 / 3.0 * eta) * xs + 113.0 / 3.0 * delta * xa;
-        m10_sigma = (-405.0 / 8.0 + 2.5 * eta) * xs * xs + (-405.0 / 8.0 + 200.0 * eta) * xa * xa -
-                    405.0 / 4.0 * delta * xs * xa;
-    }
-    const double eta2 = eta * eta;
-    const double phi2 = 3715.0 / 756.0 + 55.0 / 9.0 * eta;
-    const double phi3 = -16.0 * kPi + four_beta;
-    const double phi4 = 15293365.0 / 508032.0 + 27145.0 / 504.0 * eta + 3085.0 / 72.0 * eta2 + m10_sigma;
-    const double phi5 = kPi * (38645.0 / 756.0 - 65.0 / 9.0 * eta);
-    const double ph5l = 3.0 * phi5;
-    constexpr double k6const = 11583231236531.0 / 4694215680.0 - 640.0 / 3.0 * kPi * kPi -
-                               6848.0 / 21.0 * (kEulerG + kLn4);
-    const double phi6 = k6const + eta * (-15737765635.0 / 3048192.0 + 2255.0 / 12.0 * kPi * kPi) +
-                        76055.0 / 1728.0 * eta2 - 127825.0 / 1296.0 * eta2 * eta;
-    constexpr double ph6l = -6848.0 / 21.0;
-    const double phi7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * eta2);
-
-    // x-form, in turns: prefactor 3/(128 eta) / (2 pi); kappa^(k-5) x^(k-5)
-    const double pref = 3.0 / (128.0 * eta) / kTwoPi;
-    const double kc   = cbrt(kPi * mc * kTsun);              // (pi Mc)^(1/3): the 0PN term depends on Mc only
-    const double kc2  = kc * kc;
-    double *r = a.rec + b;
-    const int64_t S = a.rec_stride;
-    r[0 * S] = (3.0 / 128.0 / kTwoPi) / (kc2 * kc2 * kc);                       // c0  * x^-5
-    r[1 * S] = pref * phi2 / (kPi * mtot);                                      // c2  * x^-3
-    r[2 * S] = pref * phi3 * ikap * ikap;                                       // c3  * x^-2
-    r[3 * S] = pref * phi4 * ikap;                                              // c4  * x^-1
-    r[4 * S] = pref * (phi5 + ph5l * lnk) - (phic + 0.25 * kPi) / kTwoPi;       // c5  (constant)
-    r[5 * S] = pref * ph5l / 3.0;                                               // cL5 * ln f
-    r[6 * S] = pref * kap * (phi6 + ph6l * lnk);                                // c6  * x
-    r[7 * S] = pref * kap * ph6l / 3.0;                                         // cL6 * x ln f
-    r[8 * S] = pref * kap * kap * phi7;                                         // c7  * x^2
 
     // O4: Newtonian amplitude A0 = sqrt(5/24) pi^(-2/3) (Mc Tsun)^(5/6) / (D Mpc/c)
     const double u  = mc * kTsun;
     double a0 = sqrt(5.0 / 24.0) / cbrt(kPi * kPi) * (sqrt(u) * cbrt(u)) / (dl * kMpcSec);
     if (!ok) a0 = __longlong_as_double(0x7ff8000000000000LL);
 
-    // O6: sky frame (shared by all detectors)
+    // O6: sky frame
     double sg, cg, sd, cd, sp, cp;
     sincos(a.gmst - ra, &sg, &cg);
     sincos(dec, &sd, &cd);
@@ -193,12 +207,15 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
     const double n[3] = {cd * cg, -cd * sg, sd};             // cos(ra - gmst) = cg, sin(ra - gmst) = -sg
     const double pol_plus = 0.5 * (1.0 + cosi * cosi);
 
-    double tau0 = 0.0;
-    for (int i = 0; i < a.n_det; ++i) {
+    auto delay_of = [&](const DetGeom &g) {
+        return g.kind == GW_DET_FIXED ? g.dt_s : -(g.rc[0] * n[0] + g.rc[1] * n[1] + g.rc[2] * n[2]);
+    };
+    const double tau0 = tc + delay_of(a.dets.d[0]);
+    for (int i = i_first; i <= i_last; ++i) {
         const DetGeom &g = a.dets.d[i];
-        double fp, fc, dt;
+        double fp, fc;
         if (g.kind == GW_DET_FIXED) {
-            fp = g.fplus; fc = g.fcross; dt = g.dt_s;
+            fp = g.fplus; fc = g.fcross;
         } else {
             // D symmetric: (xx, xy, xz, yy, yz, zz)
             const double DX[3] = {g.D[0] * X[0] + g.D[1] * X[1] + g.D[2] * X[2],
@@ -209,11 +226,9 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
                                   g.D[2] * Y[0] + g.D[4] * Y[1] + g.D[5] * Y[2]};
             fp = (X[0] * DX[0] + X[1] * DX[1] + X[2] * DX[2]) - (Y[0] * DY[0] + Y[1] * DY[1] + Y[2] * DY[2]);
             fc = 2.0 * (X[0] * DY[0] + X[1] * DY[1] + X[2] * DY[2]);
-            dt = -(g.rc[0] * n[0] + g.rc[1] * n[1] + g.rc[2] * n[2]);
         }
-        double tau = tc + dt;
-        if (i == 0) tau0 = tau;
-        else if (a.relative_tau) tau -= tau0;
+        double tau = tc + delay_of(g);
+        if (i > 0 && a.relative_tau) tau -= tau0;
         double rc_, rs_;
         cis_turns_of_product(-a.rot_stride_hz, tau, rc_, rs_);
         double *ri = r + (int64_t)(9 + kRecPerDet * i) * S;
@@ -233,7 +248,7 @@ cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int s
     a.dets = dets; a.gmst = gmst; a.n_det = t.n_det; a.spin_order = spin_order;
     a.n_prop = n_prop; a.rec_stride = rec_stride; a.theta = theta_dev; a.rec = rec;
     a.rot_stride_hz = rot_stride_hz; a.relative_tau = relative_tau;
-    const unsigned blocks = (unsigned)((n_prop + 127) / 128);
+    const unsigned blocks = (unsigned)((n_prop + 31) / 32);
     setup_kernel<<<blocks, 128, 0, s>>>(a);
     *launches += 1;
     return cudaGetLastError();
