@@ -1,0 +1,122 @@
+"""`-m gpu`: memory safety and API-contract checks of the CUDA path that need no oracle arithmetic beyond a
+reference value (compute-sanitizer is closed on this GPU pool, so out-of-bounds writes are hunted with guard
+bands around every caller-owned output buffer)."""
+import numpy as np
+import pytest
+
+from paper_1904_02863_b200 import inputs
+
+from gpu_common import assert_lnl_close, make_ctx, make_problem
+
+pytestmark = pytest.mark.gpu
+
+GUARD = 4096          # doubles of guard band on each side
+CANARY = -7.25e300
+
+
+def _guarded(torch, n_doubles):
+    buf = torch.full((n_doubles + 2 * GUARD,), CANARY, dtype=torch.float64, device="cuda")
+    return buf, buf[GUARD:GUARD + n_doubles]
+
+
+def _intact(torch, buf, n_doubles):
+    return bool((buf[:GUARD] == CANARY).all()) and bool((buf[GUARD + n_doubles:] == CANARY).all())
+
+
+@pytest.mark.parametrize("name,red,batches", [
+    ("C1", dict(f_max=181.75, batch=600), [1, 5, 16, 33, 255, 256, 257, 600]),
+    ("C0", dict(f_max=100.0, batch=300), [1, 7, 300]),
+])
+def test_outputs_stay_inside_their_buffers(oracle, name, red, batches):
+    import torch
+    cfg = inputs.CONFIGS[name].reduced(**red)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        for B in batches:
+            thd = torch.from_numpy(th[:B]).cuda()
+            nl, npart, nh = B, B * cfg.n_det * 3, B * cfg.n_det * cfg.n_bins * 2
+            lbuf, lnl = _guarded(torch, nl)
+            pbuf, parts = _guarded(torch, npart)
+            hbuf, h = _guarded(torch, nh)
+            ctx.lnl_batch(thd, out=lnl, parts=parts.view(B, cfg.n_det, 3))
+            ctx.waveform_batch(thd, out=torch.view_as_complex(h.view(B, cfg.n_det, cfg.n_bins, 2)))
+            torch.cuda.synchronize()
+            assert _intact(torch, lbuf, nl) and _intact(torch, pbuf, npart) and _intact(torch, hbuf, nh), B
+            assert bool((lnl != CANARY).all()) and bool((parts != CANARY).all()) and bool((h != CANARY).all()), B
+
+
+def test_non_default_stream_and_two_contexts(oracle):
+    """Calls enqueue on the stream they are given; two contexts on two streams do not disturb each other."""
+    import torch
+    cfg_a = inputs.CONFIGS["C1"].reduced(f_max=150.0, batch=300)
+    cfg_b = inputs.CONFIGS["C2"].reduced(f_max=24.0, batch=90)
+    pa, pb = make_problem(oracle, cfg_a), make_problem(oracle, cfg_b)
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    with make_ctx(cfg_a, pa[0], pa[3], pa[1], pa[2]) as ca, make_ctx(cfg_b, pb[0], pb[3], pb[1], pb[2]) as cb:
+        ta, tb = torch.from_numpy(pa[4]).cuda(), torch.from_numpy(pb[4]).cuda()
+        torch.cuda.synchronize()
+        outs_a, outs_b = [], []
+        for _ in range(5):
+            with torch.cuda.stream(sa):
+                outs_a.append(ca.lnl_batch(ta, want_parts=True, stream=sa))
+            with torch.cuda.stream(sb):
+                outs_b.append(cb.lnl_batch(tb, want_parts=True, stream=sb))
+        sa.synchronize(); sb.synchronize()
+    ref_a = oracle.lnl(pa[0], cfg_a.delta_f, pa[3], pa[1], pa[2], cfg_a.gmst, pa[4], cfg_a.spin_order)
+    ref_b = oracle.lnl(pb[0], cfg_b.delta_f, pb[3], pb[1], pb[2], cfg_b.gmst, pb[4], cfg_b.spin_order)
+    for lnl, parts in outs_a:
+        assert_lnl_close(lnl.cpu().numpy(), parts.cpu().numpy(), ref_a[0], ref_a[1])
+        assert torch.equal(lnl, outs_a[0][0])
+    for lnl, parts in outs_b:
+        assert_lnl_close(lnl.cpu().numpy(), parts.cpu().numpy(), ref_b[0], ref_b[1])
+        assert torch.equal(lnl, outs_b[0][0])
+
+
+def test_reserve_growth_keeps_results(oracle):
+    """gw_ctx_reserve reallocates the workspace; results before and after are identical bits for the same plan."""
+    import torch
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=200.0, batch=1000)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    with make_ctx(cfg, f, d, S, dets, max_batch=64) as ctx:
+        thd = torch.from_numpy(th).cuda()
+        small = ctx.lnl_batch(thd[:64].contiguous()).clone()
+        ctx.reserve(1000)
+        again = ctx.lnl_batch(thd[:64].contiguous())
+        full, parts = ctx.lnl_batch(thd, want_parts=True)
+        torch.cuda.synchronize()
+        assert torch.equal(small, again)
+        ctx.reserve(10)                                   # never shrinks
+        assert ctx.info()["max_batch"] == 1000
+    ref = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th, cfg.spin_order)
+    assert_lnl_close(full.cpu().numpy(), parts.cpu().numpy(), ref[0], ref[1])
+
+
+def test_nan_rows_in_every_lane_layout(oracle):
+    """An out-of-domain proposal poisons only its own outputs, whatever the lanes-per-proposal layout."""
+    import torch
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=301.25, batch=600)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        for B in (2, 9, 40, 300, 600):
+            bad = th[:B].copy()
+            bad[B // 2, inputs.P_MC] = -3.0
+            good = ctx.lnl_batch(torch.from_numpy(th[:B]).cuda()).cpu().numpy()
+            got = ctx.lnl_batch(torch.from_numpy(bad).cuda()).cpu().numpy()
+            assert np.isnan(got[B // 2])
+            keep = np.arange(B) != B // 2
+            assert np.array_equal(got[keep], good[keep]), B
+
+
+def test_launch_count_and_plan_are_stable(oracle):
+    import torch
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=120.0, batch=64)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        n0 = ctx.launch_count()                           # precompute + norm
+        assert n0 == 2
+        thd = torch.from_numpy(th).cuda()
+        ctx.lnl_batch(thd)
+        ctx.waveform_batch(thd)
+        torch.cuda.synchronize()
+        assert ctx.launch_count() == n0 + 4               # (setup + fused) + (setup + waveform)
+        assert ctx.plan(64) == ctx.plan(64)
