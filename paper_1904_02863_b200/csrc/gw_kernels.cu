@@ -9,8 +9,9 @@
 // and the per-bin basis b = (x^-5, x^-3, x^-2, x^-1, L, x, xL, x^2),
 //     Phi'(f) = c5 + c0 b0 + c2 b1 + c3 b2 + c4 b3 + cL5 b4 + c6 b5 + cL6 b6 + c7 b7          [turns]
 // is the TaylorF2 phase WITHOUT the 2 pi f t_c term; t_c is merged with the detector delay,
-// tau_I = t_c + dt_I, and the factor exp(+2 pi i f tau_I) is applied by a Horner-style recurrence on the
-// uniform grid (fused kernel) or directly (waveform kernel).  Shares nothing with oracle/.
+// tau_I = t_c + dt_I.  The waveform kernel adds f tau_I per detector.  The fused kernel adds f tau_0 (detector
+// 0 is the time reference) and applies the remaining exp(+2 pi i f (tau_I - tau_0)), I >= 1, by a Horner-style
+// recurrence on the uniform grid.  Shares nothing with oracle/.
 #include <cmath>
 #include <cstdio>
 
@@ -404,10 +405,11 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
 // chunk; the tables are read from shared memory as warp broadcasts), 2..32 for small batches (the lanes
 // of a proposal interleave over the bins; a fixed xor-shuffle tree combines them).
 // The chunk is streamed through a kStages-deep ring of kStageBins-bin stages by bulk async copies (TMA
-// engine) completing on mbarriers.  Per (proposal, bin): 8 FMA phase, 16-op sincos, and per detector
-//     Z_I <- Z_I * rot_I + g_Ij * e^{+2 pi i Phi'_j}                                  (8 fp64 ops)
-// where rot_I = exp(-2 pi i lpp df tau_I): after the sweep Z_I * exp(+2 pi i f_last tau_I) equals
-// sum_j g_Ij exp(+2 pi i (Phi'_j + f_j tau_I)), i.e. the time shift of PAPER.md:69 costs no sincos.
+// engine) completing on mbarriers.  Per (proposal, bin): 9 FMA phase (incl. f tau_0), 16-op sincos giving
+// E = e^{+2 pi i (Phi' + f tau_0)}, detector 0: Z_0 += g_0j E (4 FMA), and per detector I >= 1
+//     Z_I <- Z_I * rot_I + g_Ij * E                                                  (8 fp64 ops)
+// where rot_I = exp(-2 pi i lpp df (tau_I - tau_0)): after the sweep Z_I * exp(+2 pi i f_last (tau_I - tau_0))
+// equals sum_j g_Ij exp(+2 pi i (Phi'_j + f_j tau_I)), i.e. the time shift of PAPER.md:69 costs no sincos.
 // <h|h>_I = |CA_I|^2 I7_I exactly for this waveform, so only <d|h> is accumulated.
 // Cross-chunk: partials to the workspace, a per-tile ticket, and the last CTA of a tile sums the chunks in
 // index order (deterministic) and writes lnL and parts.
