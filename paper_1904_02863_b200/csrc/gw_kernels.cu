@@ -289,8 +289,17 @@ __device__ __forceinline__ double phase_turns(const PhaseCoef &k, double2 b01, d
 // 16 B/element store stream.
 //     h_I(f) = CA_I f^(-7/6) exp(-2 pi i (Phi'(f) + f tau_I))
 // =====================================================================================================
-constexpr int kWfProps = 8;      // proposals per CTA
-constexpr int kWfBins  = 2;      // bins per thread (kThreads * kWfBins bins per CTA)
+#ifndef GW_WF_PROPS
+#define GW_WF_PROPS 16
+#endif
+#ifndef GW_WF_BINS
+#define GW_WF_BINS 2
+#endif
+#ifndef GW_WF_MIN_CTAS
+#define GW_WF_MIN_CTAS 1
+#endif
+constexpr int kWfProps = GW_WF_PROPS;     // proposals per CTA
+constexpr int kWfBins  = GW_WF_BINS;      // bins per thread (kThreads * kWfBins bins per CTA)
 
 struct WaveArgs {
     const double *planes, *rec;
@@ -300,7 +309,7 @@ struct WaveArgs {
 };
 
 template <int NDET>
-__global__ void __launch_bounds__(kThreads) waveform_kernel(const WaveArgs a)
+__global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(const WaveArgs a)
 {
     constexpr int NF = 10 + 4 * NDET;            // doubles per staged record: 9 coefs + pad, (tau, pad, CAre, CAim) per det
     __shared__ __align__(16) double srec[kWfProps][NF];
