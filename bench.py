@@ -175,9 +175,6 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_1904_02863_b200.csrc import build as csrc_build
-    if int(os.environ.get("LOCAL_RANK", "0")) == 0 and os.path.exists(csrc_build.NVCC):
-        csrc_build.build()             # no-op when csrc/libgwlnl.so is newer than its sources
-    from paper_1904_02863_b200 import GwContext, binding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -188,6 +185,11 @@ def run_ours(args):
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if local == 0 and os.path.exists(csrc_build.NVCC):
+        csrc_build.build()             # no-op when csrc/libgwlnl.so is newer than its sources
+    if world > 1:
+        dist.barrier()                 # nobody loads the library while local rank 0 may be rebuilding it
+    from paper_1904_02863_b200 import GwContext, binding
     n_gpus = world
 
     name, cfg, batch = parse_workload(args.workload)
@@ -298,8 +300,31 @@ def run_ours(args):
            "d2h_bytes_per_step": int(out_host.nbytes) * world, "ms_per_step": 1e3 * e2e_s / args.steps,
            "api": "gw_lnl_batch_host (pinned host theta in, host lnL out, stream synchronised)"}
 
-    # ---- the waveform-only kernel (north_star item (3)): achieved HBM GB/s ----
     extra = {}
+    # ---- small batches: latency of one call replayed from a CUDA graph (SURVEY.md 8(d) timing protocol) ----
+    if rank == 0 and B <= 256:
+        g = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        side.wait_stream(stream)
+        with torch.cuda.stream(side):
+            ctx.lnl_batch(thd, out=lnl, stream=side)
+            with torch.cuda.graph(g, stream=side):
+                ctx.lnl_batch(thd, out=lnl, stream=side)
+        stream.wait_stream(side)
+        torch.cuda.synchronize()
+        for _ in range(10):
+            g.replay()
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_rep = 200
+        g0.record(stream)
+        for _ in range(n_rep):
+            g.replay()
+        g1.record(stream)
+        torch.cuda.synchronize()
+        extra["cuda_graph_replay"] = {"ms_per_call": g0.elapsed_time(g1) / n_rep, "calls": n_rep,
+                                      "note": "back-to-back replays of one captured gw_lnl_batch, no L2 flush"}
+
+    # ---- the waveform-only kernel (north_star item (3)): achieved HBM GB/s ----
     if rank == 0 and not args.no_waveform:
         wb = min(B, max(1, int((2 << 30) // (n_det * M * 16))))
         h = torch.empty((wb, n_det, M), dtype=torch.complex128, device="cuda")
@@ -327,6 +352,8 @@ def run_ours(args):
         rate, used, n, dt, passes = oracle_rate(cfg, f, S, dets, d, th, args.cpu_seconds)
         cpu = {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle",
                "sample": f"first {n} of {B} proposals x {passes} passes, all {M} bins x {n_det} detectors, {dt:.1f} s wall"}
+        r1, u1, n1, dt1, p1 = oracle_rate(cfg, f, S, dets, d, th, min(3.0, args.cpu_seconds), n_threads=1)
+        cpu["single_thread"] = {"value": r1, "cores": u1, "sample": f"first {n1} proposals x {p1} passes, {dt1:.1f} s wall"}
 
     clocks = clk.summary()
     ctx.close()

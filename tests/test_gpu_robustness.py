@@ -120,3 +120,31 @@ def test_launch_count_and_plan_are_stable(oracle):
         torch.cuda.synchronize()
         assert ctx.launch_count() == n0 + 4               # (setup + fused) + (setup + waveform)
         assert ctx.plan(64) == ctx.plan(64)
+
+
+def test_batch_call_is_capturable_in_a_cuda_graph(oracle):
+    """The batch calls neither allocate nor synchronise nor copy (PAPER.md:45/:49 lesson), so one can be captured
+    in a CUDA graph; replays give the same bits, and follow new theta written into the captured buffer."""
+    import torch
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=150.0, batch=40)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        thd = torch.from_numpy(th).cuda()
+        out = torch.empty(40, dtype=torch.float64, device="cuda")
+        eager = ctx.lnl_batch(thd).clone()
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            ctx.lnl_batch(thd, out=out, stream=side)
+            with torch.cuda.graph(g, stream=side):
+                ctx.lnl_batch(thd, out=out, stream=side)
+        torch.cuda.current_stream().wait_stream(side)
+        out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, eager)
+        thd.copy_(torch.from_numpy(th[::-1].copy()).cuda())
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, eager.flip(0))
