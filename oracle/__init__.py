@@ -54,6 +54,14 @@ def _load():
     lib.gwo_antenna.argtypes = [dp, dbl, dbl, dbl, dbl, dp, dp, dp]
     lib.gwo_sky_frame.argtypes = [dbl, dbl, dbl, dbl, dp, dp, dp]
     lib.gwo_waveform.argtypes = [i64, dp, cint, dp, dbl, i64, dp, cint, dp]
+    lib.gwo_waveform_opt.argtypes = [i64, dp, cint, dp, dbl, i64, dp, cint, cint, dp]
+    lib.gwo_lnl_opt.argtypes = [i64, dp, dbl, cint, dp, dp, dp, dbl, i64, dp, cint, cint, cint, dp, dp]
+    lib.gwo_lnl_opt.restype = cint
+    lib.gwo_f_isco.argtypes = [dbl, dbl]
+    lib.gwo_f_isco.restype = dbl
+    lib.gwo_log_bessel_i0.argtypes = [dbl]
+    lib.gwo_log_bessel_i0.restype = dbl
+    lib.gwo_lnl_phase_marginal.argtypes = [i64, cint, dp, dp]
     lib.gwo_lnl.argtypes = [i64, dp, dbl, cint, dp, dp, dp, dbl, i64, dp, cint, cint, dp, dp]
     lib.gwo_lnl.restype = cint
     lib.gwo_inner.argtypes = [i64, dbl, dp, dp, dp, dp, dp]
@@ -127,18 +135,18 @@ def sky_frame(ra, dec, psi, gmst):
     return X, Y, n
 
 
-def waveform(freqs, dets, gmst, theta, spin_order=1) -> np.ndarray:
-    """O4..O6: h[n_prop][n_det][n_bins] complex128."""
+def waveform(freqs, dets, gmst, theta, spin_order=1, isco_cut=0) -> np.ndarray:
+    """O4..O6: h[n_prop][n_det][n_bins] complex128 (isco_cut=1: zero above f_ISCO, NEXT-1 option)."""
     f = _f64(freqs)
     d = _f64(dets).reshape(-1, DET_ROW)
     th = _f64(theta).reshape(-1, NPARAM)
     out = np.empty((th.shape[0], d.shape[0], f.shape[0], 2))
-    _load().gwo_waveform(f.shape[0], _p(f), d.shape[0], _p(d), gmst, th.shape[0], _p(th),
-                         spin_order, _p(out))
+    _load().gwo_waveform_opt(f.shape[0], _p(f), d.shape[0], _p(d), gmst, th.shape[0], _p(th),
+                             spin_order, int(isco_cut), _p(out))
     return out.view(np.complex128)[..., 0]
 
 
-def lnl(freqs, delta_f, data, psd, dets, gmst, theta, spin_order=1, n_threads=0):
+def lnl(freqs, delta_f, data, psd, dets, gmst, theta, spin_order=1, n_threads=0, isco_cut=0):
     """O7 -> (lnL[n_prop], parts[n_prop][n_det][3], threads_used)."""
     f = _f64(freqs)
     d = _f64(dets).reshape(-1, DET_ROW)
@@ -148,8 +156,8 @@ def lnl(freqs, delta_f, data, psd, dets, gmst, theta, spin_order=1, n_threads=0)
     th = _f64(theta).reshape(-1, NPARAM)
     out = np.empty(th.shape[0])
     parts = np.empty((th.shape[0], n_det, 3))
-    used = _load().gwo_lnl(n_bins, _p(f), float(delta_f), n_det, _p(dat), _p(S), _p(d), gmst,
-                           th.shape[0], _p(th), spin_order, int(n_threads), _p(out), _p(parts))
+    used = _load().gwo_lnl_opt(n_bins, _p(f), float(delta_f), n_det, _p(dat), _p(S), _p(d), gmst,
+                               th.shape[0], _p(th), spin_order, int(isco_cut), int(n_threads), _p(out), _p(parts))
     return out, parts, used
 
 
@@ -165,3 +173,21 @@ def norm_i7(freqs, delta_f, psd) -> float:
     """I7 = 4 df sum f^(-7/3)/S."""
     f, S = _f64(freqs), _f64(psd)
     return _load().gwo_norm_i7(f.shape[0], _p(f), float(delta_f), _p(S))
+
+
+def f_isco(mc: float, q: float) -> float:
+    """NEXT-1 option: 1/(6^(3/2) pi M_s)."""
+    return _load().gwo_f_isco(mc, q)
+
+
+def log_bessel_i0(x: float) -> float:
+    """ln I0(x) from the integral definition (trapezoid rule)."""
+    return _load().gwo_log_bessel_i0(float(x))
+
+
+def lnl_phase_marginal(parts) -> np.ndarray:
+    """NEXT-1 option: ln I0(|sum_I <d|h>_I|) - 1/2 sum_I <h|h>_I per proposal, from parts[n_prop][n_det][3]."""
+    p = _f64(parts)
+    out = np.empty(p.shape[0])
+    _load().gwo_lnl_phase_marginal(p.shape[0], p.shape[1], _p(p), _p(out))
+    return out

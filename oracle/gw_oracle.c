@@ -152,6 +152,17 @@ double gwo_phase(double f, const double *theta, int spin_order)
     return phase_of(&s, f);
 }
 
+/* ---- NEXT-1 option: inspiral cut-off ---------------------- */
+/* f_ISCO = 1 / (6^(3/2) pi M_s): the gravitational-wave frequency of the innermost stable circular orbit of
+ * a Schwarzschild hole of the total mass; with isco_cut the template is zero for f > f_ISCO (bins with
+ * f <= f_ISCO are kept).  Off by default (reading A6).                                                 */
+double gwo_f_isco(double mc_msun, double q)
+{
+    double eta, mtot_s, mu1, mu2;
+    gwo_masses(mc_msun, q, &eta, &mtot_s, &mu1, &mu2);
+    return 1.0 / (6.0 * sqrt(6.0) * GWO_PI * mtot_s);
+}
+
 /* ---- O4: Newtonian amplitude ------------------------------------------------------------ */
 /* A0 = sqrt(5/24) pi^(-2/3) (Mc T_sun)^(5/6) / (D Mpc/c)   [s^(-1/6)];  h0(f) = A0 f^(-7/6) exp(-i Psi). */
 double gwo_amplitude(double mc_msun, double dl_mpc)
@@ -208,8 +219,9 @@ void gwo_sky_frame(double ra, double dec, double psi, double gmst, double *X, do
 /* ---- O4..O6: detector-frame waveform at one (theta, detector, frequency) ------------------- */
 /* h_I(f) = [F+ 1/2(1+cos^2 i) - i Fx cos i] * A0 f^(-7/6) exp(-i Psi(f)) * exp(-2 pi i f dt_I) */
 static double complex h_det_at(double f, const gwo_source *src, double cosi,
-                               double a0, double fplus, double fcross, double dt_s)
+                               double a0, double fplus, double fcross, double dt_s, double f_cut)
 {
+    if (f_cut > 0.0 && f > f_cut) return 0.0;      /* NEXT-1 option isco_cut: h = 0 above f_ISCO */
     double complex h0     = a0 * pow(f, -7.0 / 6.0) * cexp(CMPLX(0.0, -phase_of(src, f)));    /* O4 */
     double complex hplus  = 0.5 * (1.0 + cosi * cosi) * h0;                 /* O5 */
     double complex hcross = CMPLX(0.0, -cosi) * h0;                         /* O5 */
@@ -218,20 +230,21 @@ static double complex h_det_at(double f, const gwo_source *src, double cosi,
 }
 
 /* h_out[n_prop][n_det][n_bins][2] (re, im) */
-void gwo_waveform(int64_t n_bins, const double *freqs, int n_det, const double *dets, double gmst,
-                  int64_t n_prop, const double *theta, int spin_order, double *h_out)
+void gwo_waveform_opt(int64_t n_bins, const double *freqs, int n_det, const double *dets, double gmst,
+                      int64_t n_prop, const double *theta, int spin_order, int isco_cut, double *h_out)
 {
 #pragma omp parallel for schedule(dynamic, 1)
     for (int64_t b = 0; b < n_prop; ++b) {
         const double *th = theta + b * T_N;
         const double a0 = gwo_amplitude(th[T_MC], th[T_DL]);
         const gwo_source src = source_of(th, spin_order);
+        const double f_cut = isco_cut ? gwo_f_isco(th[T_MC], th[T_Q]) : 0.0;
         for (int i = 0; i < n_det; ++i) {
             double fp, fc, dt;
             gwo_antenna(dets + (size_t)i * D_N, th[T_RA], th[T_DEC], th[T_PSI], gmst, &fp, &fc, &dt);
             double *row = h_out + (((size_t)b * n_det + i) * (size_t)n_bins) * 2;
             for (int64_t j = 0; j < n_bins; ++j) {
-                double complex h = h_det_at(freqs[j], &src, th[T_COSI], a0, fp, fc, dt);
+                double complex h = h_det_at(freqs[j], &src, th[T_COSI], a0, fp, fc, dt, f_cut);
                 row[2 * j]     = creal(h);
                 row[2 * j + 1] = cimag(h);
             }
@@ -252,10 +265,10 @@ static void neumaier_add(double *sum, double *comp, double x)
 /* data_ri[n_det][n_bins][2], psd[n_det][n_bins]; lnl[n_prop]; parts[n_prop][n_det][3] =
  * (Re<d|h>, Im<d|h>, <h|h>) (parts may be NULL).  n_threads <= 0: OpenMP default.
  * Returns the number of threads the proposal loop used.                                        */
-int gwo_lnl(int64_t n_bins, const double *freqs, double delta_f, int n_det,
-            const double *data_ri, const double *psd, const double *dets, double gmst,
-            int64_t n_prop, const double *theta, int spin_order, int n_threads,
-            double *lnl, double *parts)
+int gwo_lnl_opt(int64_t n_bins, const double *freqs, double delta_f, int n_det,
+                const double *data_ri, const double *psd, const double *dets, double gmst,
+                int64_t n_prop, const double *theta, int spin_order, int isco_cut, int n_threads,
+                double *lnl, double *parts)
 {
     int used = 1;
 #ifdef _OPENMP
@@ -268,6 +281,7 @@ int gwo_lnl(int64_t n_bins, const double *freqs, double delta_f, int n_det,
         const double *th = theta + b * T_N;
         const double a0 = gwo_amplitude(th[T_MC], th[T_DL]);
         const gwo_source src = source_of(th, spin_order);
+        const double f_cut = isco_cut ? gwo_f_isco(th[T_MC], th[T_Q]) : 0.0;
         double total = 0.0;
         for (int i = 0; i < n_det; ++i) {
             double fp, fc, dt;
@@ -276,7 +290,7 @@ int gwo_lnl(int64_t n_bins, const double *freqs, double delta_f, int n_det,
             const double *S = psd + (size_t)i * (size_t)n_bins;
             double dh_re = 0, dh_re_c = 0, dh_im = 0, dh_im_c = 0, hh = 0, hh_c = 0;
             for (int64_t j = 0; j < n_bins; ++j) {
-                double complex h  = h_det_at(freqs[j], &src, th[T_COSI], a0, fp, fc, dt);
+                double complex h  = h_det_at(freqs[j], &src, th[T_COSI], a0, fp, fc, dt, f_cut);
                 double complex dj = CMPLX(d[2 * j], d[2 * j + 1]);
                 double complex t  = dj * conj(h) / S[j];
                 neumaier_add(&dh_re, &dh_re_c, creal(t));
@@ -295,6 +309,56 @@ int gwo_lnl(int64_t n_bins, const double *freqs, double delta_f, int n_det,
         lnl[b] = total;
     }
     return used;
+}
+
+/* the default (no cut-off) entry points, as pinned by tests/test_oracle_*.py */
+void gwo_waveform(int64_t n_bins, const double *freqs, int n_det, const double *dets, double gmst,
+                  int64_t n_prop, const double *theta, int spin_order, double *h_out)
+{
+    gwo_waveform_opt(n_bins, freqs, n_det, dets, gmst, n_prop, theta, spin_order, 0, h_out);
+}
+int gwo_lnl(int64_t n_bins, const double *freqs, double delta_f, int n_det,
+            const double *data_ri, const double *psd, const double *dets, double gmst,
+            int64_t n_prop, const double *theta, int spin_order, int n_threads,
+            double *lnl, double *parts)
+{
+    return gwo_lnl_opt(n_bins, freqs, delta_f, n_det, data_ri, psd, dets, gmst, n_prop, theta, spin_order, 0,
+                       n_threads, lnl, parts);
+}
+
+/* ---- NEXT-1 option: likelihood marginalised over the coalescence phase --------------------------------- */
+/* h depends on phi_c only through the factor exp(+i phi_c) (O3/O4), so with a uniform prior on phi_c
+ *   L_marg = (1/2 pi) int_0^{2 pi} exp( Re[ e^{-i phi} sum_I <d|h>_I ] - 1/2 sum_I <h|h>_I ) d phi
+ *          = I0(|sum_I <d|h>_I|) exp(-1/2 sum_I <h|h>_I),
+ * where <d|h>_I is evaluated at any phi_c.  ln I0 is computed from its integral definition
+ *   I0(x) = (1/pi) int_0^pi exp(x cos t) dt  =>  ln I0(x) = x + ln[(1/pi) int_0^pi exp(x (cos t - 1)) dt]
+ * by the trapezoid rule on n points (exponentially convergent for this periodic, even integrand; n is chosen
+ * from x so that the Gaussian peak of width ~1/sqrt(x) is resolved).                                       */
+double gwo_log_bessel_i0(double x)
+{
+    x = fabs(x);
+    long n = 64 + (long)(64.0 * sqrt(x));                 /* >= 64 points per peak width */
+    if (n > 4000000) n = 4000000;
+    double s = 0, c = 0;
+    for (long k = 0; k <= n; ++k) {
+        double t = GWO_PI * (double)k / (double)n;
+        double w = (k == 0 || k == n) ? 0.5 : 1.0;
+        neumaier_add(&s, &c, w * exp(x * (cos(t) - 1.0)));
+    }
+    return x + log((s + c) / (double)n);
+}
+
+/* lnl_marg[b] = ln I0(|sum_I (parts[b][I][0] + i parts[b][I][1])|) - 1/2 sum_I parts[b][I][2] */
+void gwo_lnl_phase_marginal(int64_t n_prop, int n_det, const double *parts, double *lnl_marg)
+{
+    for (int64_t b = 0; b < n_prop; ++b) {
+        double re = 0, im = 0, hh = 0;
+        for (int i = 0; i < n_det; ++i) {
+            const double *p = parts + ((size_t)b * n_det + i) * 3;
+            re += p[0]; im += p[1]; hh += p[2];
+        }
+        lnl_marg[b] = gwo_log_bessel_i0(hypot(re, im)) - 0.5 * hh;
+    }
 }
 
 /* generic noise-weighted inner product <a|b> = 4 df sum a conj(b)/S for one detector (pins P3) */
