@@ -200,7 +200,8 @@ def run_ours(args):
     B, M, n_det = len(th), cfg.n_bins, cfg.n_det
     stream = torch.cuda.current_stream()
 
-    ctx = GwContext(f, d, S, dets, cfg.gmst, spin_order=cfg.spin_order, max_batch=B)
+    ctx = GwContext(f, d, S, dets, cfg.gmst, spin_order=cfg.spin_order, max_batch=B,
+                    isco_cut=int(args.isco_cut), phase_marginal=int(args.phase_marginal))
     thd = torch.from_numpy(th).cuda()
     lnl = torch.empty(B, dtype=torch.float64, device="cuda")
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
@@ -363,7 +364,8 @@ def run_ours(args):
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": f"{name}: {n_det} det x {M} bins x {B} proposals per GPU",
                            "global_batch": B * world, "bins": M, "detectors": n_det, "parallelism": f"proposals sharded x{world}",
-                           "l2": "flushed before every timed step: 256 MiB write, then a 256 MiB read of a second buffer (no dirty lines left)", "plan": plan},
+                           "l2": "flushed before every timed step: 256 MiB write, then a 256 MiB read of a second buffer (no dirty lines left)", "plan": plan,
+                           "options": {"isco_cut": int(args.isco_cut), "phase_marginal": int(args.phase_marginal)}},
                 "bin_det_proposals_per_s": value * M * n_det,
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
                 "roofline": roofline, "cpu_baseline": cpu}
@@ -383,6 +385,8 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-waveform", action="store_true")
+    ap.add_argument("--isco-cut", action="store_true", help="NEXT-1 option: h = 0 above f_ISCO (not the headline config)")
+    ap.add_argument("--phase-marginal", action="store_true", help="NEXT-1 option: lnL marginalised over phi_c")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -46,7 +46,7 @@
 extern "C" {
 #endif
 
-#define GW_ABI_VERSION 1
+#define GW_ABI_VERSION 2
 
 enum {
     GW_OK              =  0,
@@ -71,10 +71,16 @@ typedef struct gw_detector {
     double fplus, fcross, dt_s;  /* FIXED: response and time delay (seconds)                              */
 } gw_detector;
 
-typedef struct gw_options {      /* NULL => { spin_order 1, isco_cut 0, max_batch 4096 }                  */
+typedef struct gw_options {      /* NULL => { spin_order 1, isco_cut 0, max_batch 4096, phase_marginal 0 } */
     int     spin_order;          /* 0: no spin terms; 1: 1.5PN spin-orbit + 2PN spin-spin (A7)  */
-    int     isco_cut;            /* must be 0 (A6: every bin of the band is evaluated)          */
+    int     isco_cut;            /* 0 (default, A6): every bin of the band is evaluated;
+                                    1 (NEXT-1 option): h = 0 for f > f_ISCO =
+                                    1/(6^(3/2) pi M) of the proposal's total mass                         */
     int64_t max_batch;           /* workspace reservation in proposals (>= 1); grow with gw_ctx_reserve   */
+    int     phase_marginal;      /* 0: lnL at the proposal's phi_c; 1 (NEXT-1 option): lnl_out holds the
+                                    likelihood marginalised over phi_c with a uniform prior,
+                                    ln I0(|sum_I <d|h>_I|) - 1/2 sum_I <h|h>_I; parts are unchanged        */
+    int     reserved;            /* must be 0                                                              */
 } gw_options;
 
 /* Column order of one proposal theta[GW_NPARAM] (units: Msun, -, -, -, Mpc, s, rad, -, rad, rad, rad):

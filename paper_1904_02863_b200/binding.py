@@ -41,7 +41,8 @@ class gw_detector(ctypes.Structure):
 
 
 class gw_options(ctypes.Structure):
-    _fields_ = [("spin_order", ctypes.c_int), ("isco_cut", ctypes.c_int), ("max_batch", ctypes.c_int64)]
+    _fields_ = [("spin_order", ctypes.c_int), ("isco_cut", ctypes.c_int), ("max_batch", ctypes.c_int64),
+                ("phase_marginal", ctypes.c_int), ("reserved", ctypes.c_int)]
 
 
 def lib_path() -> str:
@@ -132,7 +133,7 @@ class GwContext:
     """
 
     def __init__(self, freqs, data, psd, det_rows, gmst: float, spin_order: int = 1,
-                 max_batch: int = 4096, stream=None):
+                 max_batch: int = 4096, stream=None, isco_cut: int = 0, phase_marginal: int = 0):
         self._h = ctypes.c_void_p()
         self._lib = load_library()
         self._keep = []
@@ -143,7 +144,7 @@ class GwContext:
         s_ptr, n_s = self._as_ptr(psd, np.float64)
         if n_d != self.n_det * n_bins or n_s != self.n_det * n_bins:
             raise GwError(GW_ERR_INVALID_ARG, "GwContext", "data/psd must be [n_det][n_bins]")
-        opt = gw_options(int(spin_order), 0, int(max_batch))
+        opt = gw_options(int(spin_order), int(isco_cut), int(max_batch), int(phase_marginal), 0)
         rc = self._lib.gw_ctx_create(ctypes.byref(self._h), n_bins, f_ptr, self.n_det, d_ptr, s_ptr, dets,
                                      float(gmst), ctypes.byref(opt), _stream_ptr(stream))
         self._keep = []

@@ -125,7 +125,7 @@ int reserve_impl(gw_ctx *ctx, int64_t max_batch)
     w.max_batch = max_batch;
     w.rec_stride = (max_batch + 31) / 32 * 32;
     const int n_det = ctx->t.n_det;
-    const int64_t n_rec = 9 + kRecPerDet * n_det;
+    const int64_t n_rec = rec_fields(n_det);
     w.partial_doubles = need_partial > 0 ? need_partial : 1;
     w.n_tickets = need_tickets;
     w.h_stage_doubles = 0;                                    // the host waveform variant allocates its slab on first use
@@ -192,9 +192,11 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
     if (!freqs_hz || !data_ri || !psd || !dets) return GW_ERR_INVALID_ARG;
     if (n_bins < 2 || n_bins > ((int64_t)1 << 30) || n_det < 1 || n_det > GW_MAX_DET) return GW_ERR_INVALID_ARG;
     if (!std::isfinite(gmst_rad)) return GW_ERR_INVALID_ARG;
-    gw_options o = {1, 0, 4096};
+    gw_options o = {1, 0, 4096, 0, 0};
     if (opt) o = *opt;
-    if (o.spin_order < 0 || o.spin_order > 1 || o.isco_cut != 0 || o.max_batch < 1) return GW_ERR_INVALID_ARG;
+    if (o.spin_order < 0 || o.spin_order > 1 || o.isco_cut < 0 || o.isco_cut > 1 || o.max_batch < 1 ||
+        o.phase_marginal < 0 || o.phase_marginal > 1 || o.reserved != 0)
+        return GW_ERR_INVALID_ARG;
 
     cudaStream_t s = (cudaStream_t)cuda_stream;
     int dev = 0;
@@ -261,11 +263,13 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
     double *dfreq = nullptr, *ddata = nullptr, *dpsd = nullptr, *di7 = nullptr;
     Tables &t = ctx->t;
     t.n_bins = n_bins; t.n_pad = (n_bins + 31) / 32 * 32 + 32; t.n_det = n_det; t.f0 = f0; t.delta_f = df;
+    t.isco_cut = o.isco_cut; t.phase_marginal = o.phase_marginal;
     do {
         if ((e = configure_kernels(nullptr)) != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
         ctx->ctas_per_sm = fused_ctas_per_sm(n_det);
         bool ok = true;
         ok = ok && (e = cudaMalloc(&t.planes, sizeof(double) * 2 * (kBasisPlanes + n_det) * t.n_pad)) == cudaSuccess;
+        if (t.isco_cut) ok = ok && (e = cudaMalloc(&t.i7cum, sizeof(double) * n_det * t.n_pad)) == cudaSuccess;
         ok = ok && (e = cudaMalloc(&dfreq, sizeof(double) * nf)) == cudaSuccess;
         ok = ok && (e = cudaMalloc(&ddata, sizeof(double) * nd * 2)) == cudaSuccess;
         ok = ok && (e = cudaMalloc(&dpsd, sizeof(double) * nd)) == cudaSuccess;
@@ -301,7 +305,7 @@ int gw_ctx_destroy(gw_ctx *ctx)
     if (!ctx) return GW_OK;
     cudaDeviceSynchronize();
     free_workspace(ctx->w);
-    cudaFree(ctx->t.planes);
+    cudaFree(ctx->t.planes); cudaFree(ctx->t.i7cum);
     for (int i = 0; i < 3; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     delete ctx;
     cudaGetLastError();

@@ -33,6 +33,11 @@ constexpr int kBasis      = 8;     // per-bin phase basis values (4 planes of 2)
 constexpr int kBasisPlanes = 5;    // (x^-5,x^-3) (x^-2,x^-1) (ln f,x) (x ln f,x^2) (f,f^-7/6)
 constexpr int kRecFixed   = 10;    // record fields before the per-detector block
 constexpr int kRecPerDet  = 5;     // tau, Cre, Cim, rot_re, rot_im
+// record fields: 0..8 phase coefficients, then kRecPerDet per detector, then f_ISCO and the index of the last
+// bin with f_j <= f_ISCO (as a double)
+__host__ __device__ constexpr int rec_field_fisco(int n_det) { return 9 + kRecPerDet * n_det; }
+__host__ __device__ constexpr int rec_field_jcut(int n_det)  { return 10 + kRecPerDet * n_det; }
+__host__ __device__ constexpr int rec_fields(int n_det)      { return 11 + kRecPerDet * n_det; }
 
 // One detector as the kernels see it (built on the host from gw_detector).
 struct DetGeom {
@@ -51,6 +56,8 @@ struct Tables {
     double  f0, delta_f;
     double *planes;       // [5 + n_det][n_pad][2]: the five basis planes above, then g_I (re,im) per detector
     double  i7[GW_MAX_DET];   // host copy of I7_I = sum_j (4 df/S_Ij) f_j^(-7/3)
+    double *i7cum;        // isco_cut only: [n_det][n_pad] inclusive prefix sums of (4 df/S_Ij) f_j^(-7/3)
+    int     isco_cut, phase_marginal;
 };
 
 // Launch shape of one gw_lnl_batch call (a pure function of n_prop and the context; fixes summation order).

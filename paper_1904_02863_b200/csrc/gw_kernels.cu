@@ -84,6 +84,37 @@ __global__ void __launch_bounds__(1024) norm_kernel(int64_t n_bins, double delta
     if (threadIdx.x == 0) i7[i] = sh[0];
 }
 
+// isco_cut only: inclusive prefix sums cum[i][j] = sum_{k <= j} (4 df / S_Ik) f_k^(-7/3).  One CTA per detector;
+// each thread sums a contiguous slice, the slice totals are scanned in thread order by one thread, and the
+// slice is swept again: the order of additions is fixed by (M, 1024) alone.
+__global__ void __launch_bounds__(1024) norm_cum_kernel(int64_t n_bins, int64_t n_pad, double delta_f,
+                                                        const double *__restrict__ psd,
+                                                        const double2 *__restrict__ f_amp, double *__restrict__ cum)
+{
+    __shared__ double sh[1024];
+    const int i = blockIdx.x, t = threadIdx.x;
+    const int64_t len = (n_bins + 1023) / 1024;
+    const int64_t lo = (int64_t)t * len, hi = (lo + len < n_bins) ? lo + len : n_bins;
+    double s = 0.0;
+    for (int64_t j = lo; j < hi; ++j) {
+        const double a = f_amp[j].y;
+        s += (4.0 * delta_f / psd[(int64_t)i * n_bins + j]) * (a * a);
+    }
+    sh[t] = s;
+    __syncthreads();
+    if (t == 0) {
+        double run = 0.0;
+        for (int k = 0; k < 1024; ++k) { const double v = sh[k]; sh[k] = run; run += v; }   // exclusive scan
+    }
+    __syncthreads();
+    double run = sh[t];
+    for (int64_t j = lo; j < hi; ++j) {
+        const double a = f_amp[j].y;
+        run += (4.0 * delta_f / psd[(int64_t)i * n_bins + j]) * (a * a);
+        cum[(int64_t)i * n_pad + j] = run;
+    }
+}
+
 cudaError_t launch_precompute(const Tables &t, const double *freqs_dev, const double *data_dev,
                               const double *psd_dev, double *i7_dev, cudaStream_t s, int64_t *launches)
 {
@@ -96,6 +127,13 @@ cudaError_t launch_precompute(const Tables &t, const double *freqs_dev, const do
     norm_kernel<<<t.n_det, 1024, 0, s>>>(t.n_bins, t.delta_f, psd_dev,
                                          reinterpret_cast<const double2 *>(t.planes) + 4 * t.n_pad, i7_dev);
     *launches += 2;
+    if (t.isco_cut) {
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        norm_cum_kernel<<<t.n_det, 1024, 0, s>>>(t.n_bins, t.n_pad, t.delta_f, psd_dev,
+                                                 reinterpret_cast<const double2 *>(t.planes) + 4 * t.n_pad, t.i7cum);
+        *launches += 1;
+    }
     return cudaGetLastError();
 }
 
@@ -116,6 +154,9 @@ struct SetupArgs {
     double *rec;
     double  rot_stride_hz;
     int     relative_tau;     // 1: tau_I (I >= 1) and rot_I are relative to detector 0 (fused kernel); 0: absolute
+    const double2 *f_amp;     // basis plane 4: (f_j, f_j^-7/6), for the f_ISCO bin search
+    int64_t n_bins;
+    double  f0, delta_f;
 };
 
 // A CTA of 128 threads serves 32 proposals; warp w takes role w for proposal (block*32 + lane), so the four
@@ -178,6 +219,16 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
         r[6 * S] = pref * kap * (phi6 + ph6l * lnk);                                // c6  * x
         r[7 * S] = pref * kap * ph6l / 3.0;                                         // cL6 * x ln f
         r[8 * S] = pref * kap * kap * phi7;                                         // c7  * x^2
+        // NEXT-1 option isco_cut: f_ISCO = 1/(6^(3/2) pi M) and the last bin with f_j <= f_ISCO (-1: none).
+        // The decision is taken in fp64 against the same f_j the oracle compares with.
+        const double f_isco = 1.0 / (6.0 * sqrt(6.0) * (kap * kap * kap));         // kappa^3 = pi M
+        double jc = floor((f_isco - a.f0) / a.delta_f);
+        int64_t j = jc < -1.0 ? -1 : (jc > (double)(a.n_bins - 1) ? a.n_bins - 1 : (int64_t)jc);
+        while (j + 1 < a.n_bins && a.f_amp[j + 1].x <= f_isco) ++j;
+        while (j >= 0 && a.f_amp[j].x > f_isco) --j;
+        if (!(f_isco == f_isco)) j = -1;                                            // NaN masses: nothing kept
+        r[(int64_t)rec_field_fisco(a.n_det) * S] = f_isco;
+        r[(int64_t)rec_field_jcut(a.n_det) * S]  = (double)j;
         return;
     }
 
@@ -249,6 +300,8 @@ cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int s
     a.dets = dets; a.gmst = gmst; a.n_det = t.n_det; a.spin_order = spin_order;
     a.n_prop = n_prop; a.rec_stride = rec_stride; a.theta = theta_dev; a.rec = rec;
     a.rot_stride_hz = rot_stride_hz; a.relative_tau = relative_tau;
+    a.f_amp = reinterpret_cast<const double2 *>(t.planes) + 4 * t.n_pad;
+    a.n_bins = t.n_bins; a.f0 = t.f0; a.delta_f = t.delta_f;
     const unsigned blocks = (unsigned)((n_prop + 31) / 32);
     setup_kernel<<<blocks, 128, 0, s>>>(a);
     *launches += 1;
@@ -304,7 +357,7 @@ constexpr int kWfBins  = GW_WF_BINS;      // bins per thread (kThreads * kWfBins
 struct WaveArgs {
     const double *planes, *rec;
     int64_t n_pad, n_bins, n_prop, rec_stride;
-    int     bin_blocks;
+    int     bin_blocks, isco_cut;
     double *h;
 };
 
@@ -338,7 +391,8 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
         const int p = idx / NF, fld = idx % NF;
         double v = 0.0;
         if (fld < 9) v = a.rec[(int64_t)fld * a.rec_stride + b0 + p];
-        else if (fld >= 10) {
+        else if (fld == 9) v = a.isco_cut ? a.rec[(int64_t)rec_field_fisco(NDET) * a.rec_stride + b0 + p] : 1.0e308;
+        else {
             const int i = (fld - 10) >> 2, w = (fld - 10) & 3;          // w: 0 tau, 2 CAre, 3 CAim
             if (w != 1) v = a.rec[(int64_t)(9 + kRecPerDet * i + (w == 0 ? 0 : w - 1)) * a.rec_stride + b0 + p];
         }
@@ -355,6 +409,7 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
         double ph[kWfBins];
 #pragma unroll
         for (int u = 0; u < kWfBins; ++u) ph[u] = phase_turns(k, b01[u], b23[u], b45[u], b67[u]);
+        const double f_cut = k8.y;                                       // f_ISCO, or 1e308 without the cut-off
         double2 *row = h + ((b0 + p) * NDET) * a.n_bins;
 #pragma unroll
         for (int i = 0; i < NDET; ++i) {
@@ -365,7 +420,8 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
                 cis_turns(__fma_rn(f[u], t_.x, ph[u]), c, s);
                 const double kr = ca.x * amp[u], ki = ca.y * amp[u];
                 // (kr + i ki)(c - i s)
-                const double2 out = make_double2(__fma_rn(kr, c, ki * s), __fma_rn(ki, c, -(kr * s)));
+                double2 out = make_double2(__fma_rn(kr, c, ki * s), __fma_rn(ki, c, -(kr * s)));
+                if (f[u] > f_cut) out = make_double2(0.0, 0.0);            // NEXT-1 option isco_cut
                 if (in[u]) __stcs(row + j[u], out);
             }
             row += a.n_bins;
@@ -392,6 +448,7 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
     a.planes = t.planes; a.rec = rec;
     a.n_pad = t.n_pad; a.n_bins = t.n_bins; a.n_prop = n_prop; a.rec_stride = rec_stride;
     a.bin_blocks = (int)((t.n_bins + kThreads * kWfBins - 1) / (kThreads * kWfBins));
+    a.isco_cut = t.isco_cut;
     a.h = h_out;
     const int64_t p_blocks = (n_prop + kWfProps - 1) / kWfProps;
     const int64_t blocks = p_blocks * a.bin_blocks;
@@ -429,33 +486,51 @@ struct FusedArgs {
     int     n_chunks, lpp;
     double  f0, delta_f;
     double  i7[GW_MAX_DET];
+    const double *i7cum;     // isco_cut: [NDET][n_pad] prefix sums of the norm
+    int     phase_marginal;
     double *partial;
     unsigned int *tickets;
     double *lnl, *parts;
 };
 
-template <int NDET>
+// ln I0(x), x >= 0: library I0 up to 500, then the asymptotic series e^x/sqrt(2 pi x) (1 + 1/8x + 9/128x^2 + ...)
+// whose 8-term truncation error is below 1e-20 there.
+__device__ __forceinline__ double log_bessel_i0(double x)
+{
+    if (x < 500.0) return log(cyl_bessel_i0(x));
+    const double y = 1.0 / x;
+    double s = 1.0 + y * (0.125 + y * (0.0703125 + y * (0.0732421875 + y * (0.112152099609375 +
+               y * (0.22710800170898438 + y * (0.5725014209747314 + y * 1.7277275025844574))))));
+    return x - 0.5 * log(kTwoPi * x) + log(s);
+}
+
+template <int NDET, bool ISCO>
 __device__ __forceinline__ void finish_proposal(const FusedArgs &a, int64_t b, const double (&zr)[NDET],
                                                 const double (&zi)[NDET])
 {
-    double lnl = 0.0;
+    double lnl = 0.0, sum_re = 0.0, sum_im = 0.0, sum_hh = 0.0;
+    int64_t jcut = 0;
+    if (ISCO) jcut = (int64_t)a.rec[(int64_t)rec_field_jcut(NDET) * a.rec_stride + b];
 #pragma unroll
     for (int i = 0; i < NDET; ++i) {
         const double *ri = a.rec + (int64_t)(9 + kRecPerDet * i) * a.rec_stride + b;
         const double car = ri[a.rec_stride], cai = ri[2 * a.rec_stride];
         const double dh_re = __fma_rn(car, zr[i], cai * zi[i]);      // conj(CA) * Z
         const double dh_im = __fma_rn(car, zi[i], -(cai * zr[i]));
-        const double hh    = __fma_rn(car, car, cai * cai) * a.i7[i];
+        const double norm  = ISCO ? (jcut >= 0 ? a.i7cum[(int64_t)i * a.n_pad + jcut] : 0.0) : a.i7[i];
+        const double hh    = __fma_rn(car, car, cai * cai) * norm;
         lnl += dh_re - 0.5 * hh;
+        sum_re += dh_re; sum_im += dh_im; sum_hh += hh;
         if (a.parts) {
             double *p = a.parts + (b * NDET + i) * 3;
             p[0] = dh_re; p[1] = dh_im; p[2] = hh;
         }
     }
+    if (a.phase_marginal) lnl = log_bessel_i0(hypot(sum_re, sum_im)) - 0.5 * sum_hh;   // NEXT-1 option
     a.lnl[b] = lnl;
 }
 
-template <int NDET, bool MULTI>
+template <int NDET, bool MULTI, bool ISCO>
 __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedArgs a)
 {
     constexpr int NP = kBasisPlanes + NDET;                  // planes per stage
@@ -512,6 +587,8 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
         zr[i] = 0.0; zi[i] = 0.0;
     }
 
+    int64_t jcut = 0;
+    if (ISCO) jcut = (int64_t)a.rec[(int64_t)rec_field_jcut(NDET) * a.rec_stride + b];
     int iters_total = 0;
     for (int s = 0; s < n_stage; ++s) {
         const int buf = s % kStages;
@@ -519,6 +596,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
         mbar_wait(&bars[buf], (uint32_t)((s / kStages) & 1));
         const double2 *P = sm + (size_t)buf * NP * kStageBins;
         const int iters = MULTI ? (cnt + lpp - 1) / lpp : cnt;
+        const int64_t jstage = j0 + (int64_t)s * kStageBins;  // global index of the stage's first bin
         int it = 0;
         if (!MULTI) {
             // kUnroll bins per trip, written plane by plane ("k-major"): consecutive fp64 instructions then
@@ -560,6 +638,11 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                 }
 #pragma unroll
                 for (int u = 0; u < kUnroll; ++u) cis_turns(ph[u], cs[u], sn[u]);
+                if (ISCO) {                                      // h = 0 above f_ISCO: the bin contributes nothing
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u)
+                        if (jstage + it + u > jcut) { cs[u] = 0.0; sn[u] = 0.0; }
+                }
 #pragma unroll
                 for (int u = 0; u < kUnroll; ++u) {              // bins in ascending order: the Z recurrence
 #pragma unroll
@@ -592,6 +675,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             ph = __fma_rn(tau[0], P[4 * kStageBins + jj].x, ph);
             double c, sn;
             cis_turns(ph, c, sn);
+            if (ISCO && jstage + jj > jcut) { c = 0.0; sn = 0.0; }
 #pragma unroll
             for (int i = 0; i < NDET; ++i) {
                 double2 g = P[(kBasisPlanes + i) * kStageBins + jj];
@@ -638,7 +722,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
     }
 
     if (a.n_chunks == 1) {
-        if (sub == 0 && live) finish_proposal<NDET>(a, b, zr, zi);
+        if (sub == 0 && live) finish_proposal<NDET, ISCO>(a, b, zr, zi);
         return;
     }
     // stage 1 -> workspace: partial[((tile*n_chunks + chunk)*2*NDET + comp)*PT + pic]
@@ -687,7 +771,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                     si[i] += __ldcg(base + ((int64_t)c * 2 * NDET + 2 * i + 1) * PT);
                 }
             }
-            finish_proposal<NDET>(a, bb, sr, si);
+            finish_proposal<NDET, ISCO>(a, bb, sr, si);
         }
     }
     if (tid == 0) a.tickets[tile] = 0u;                      // self-reset for the next call
@@ -698,7 +782,7 @@ size_t fused_smem_bytes(int n_det)
     return (size_t)kStages * (kBasisPlanes + n_det) * kStageBins * sizeof(double2) + kStages * sizeof(uint64_t);
 }
 
-template <int NDET, bool MULTI>
+template <int NDET, bool MULTI, bool ISCO>
 static cudaError_t launch_fused_t(const FusedArgs &a, int64_t blocks, cudaStream_t s)
 {
     cudaLaunchConfig_t cfg = {};
@@ -708,7 +792,7 @@ static cudaError_t launch_fused_t(const FusedArgs &a, int64_t blocks, cudaStream
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, fused_kernel<NDET, MULTI>, a);
+    return cudaLaunchKernelEx(&cfg, fused_kernel<NDET, MULTI, ISCO>, a);
 }
 
 cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, const double *rec,
@@ -723,14 +807,23 @@ cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, cons
     const int64_t blocks = plan.n_tiles * plan.n_chunks;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     *launches += 1;
-    const bool multi = plan.lpp > 1;
+    a.i7cum = t.i7cum; a.phase_marginal = t.phase_marginal;
+    const int variant = (plan.lpp > 1 ? 1 : 0) + (t.isco_cut ? 2 : 0);
+#define GW_DISPATCH(N)                                                                      \
+    switch (variant) {                                                                      \
+    case 0: return launch_fused_t<N, false, false>(a, blocks, s);                           \
+    case 1: return launch_fused_t<N, true, false>(a, blocks, s);                            \
+    case 2: return launch_fused_t<N, false, true>(a, blocks, s);                            \
+    default: return launch_fused_t<N, true, true>(a, blocks, s);                            \
+    }
     switch (t.n_det) {
-    case 1: return multi ? launch_fused_t<1, true>(a, blocks, s) : launch_fused_t<1, false>(a, blocks, s);
-    case 2: return multi ? launch_fused_t<2, true>(a, blocks, s) : launch_fused_t<2, false>(a, blocks, s);
-    case 3: return multi ? launch_fused_t<3, true>(a, blocks, s) : launch_fused_t<3, false>(a, blocks, s);
-    case 4: return multi ? launch_fused_t<4, true>(a, blocks, s) : launch_fused_t<4, false>(a, blocks, s);
+    case 1: GW_DISPATCH(1)
+    case 2: GW_DISPATCH(2)
+    case 3: GW_DISPATCH(3)
+    case 4: GW_DISPATCH(4)
     default: return cudaErrorInvalidValue;
     }
+#undef GW_DISPATCH
 }
 
 static int g_ctas_per_sm[GW_MAX_DET + 1] = {0, 0, 0, 0, 0};
@@ -740,12 +833,16 @@ static cudaError_t configure_one()
 {
     const int smem = (int)fused_smem_bytes(NDET);
     cudaError_t e;
-    e = cudaFuncSetAttribute(fused_kernel<NDET, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    e = cudaFuncSetAttribute(fused_kernel<NDET, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(fused_kernel<NDET, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    e = cudaFuncSetAttribute(fused_kernel<NDET, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fused_kernel<NDET, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fused_kernel<NDET, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     int n = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fused_kernel<NDET, false>, kThreads, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fused_kernel<NDET, false, false>, kThreads, smem);
     if (e != cudaSuccess) return e;
     g_ctas_per_sm[NDET] = n > 0 ? n : 1;
     return cudaSuccess;
