@@ -148,3 +148,26 @@ def test_batch_call_is_capturable_in_a_cuda_graph(oracle):
         g.replay()
         torch.cuda.synchronize()
         assert torch.equal(out, eager.flip(0))
+
+
+def test_sub_band_contexts_add_up(oracle):
+    """Bin sharding (sharding.bin_shard_edges): contexts built on contiguous sub-bands give parts whose sum is the
+    full-band result (what a bin-sharded multi-GPU run exchanges)."""
+    import torch
+    from paper_1904_02863_b200 import GwContext
+    from paper_1904_02863_b200.sharding import bin_shard_edges, lnl_from_parts
+    cfg = inputs.CONFIGS["C2"].reduced(f_max=30.0, batch=48)              # 1281 bins
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    thd = torch.from_numpy(th).cuda()
+    total = None
+    for lo, hi in bin_shard_edges(cfg.n_bins, 3):
+        with GwContext(f[lo:hi], d[:, lo:hi], S[:, lo:hi], dets, cfg.gmst, max_batch=48) as ctx:
+            _, parts = ctx.lnl_batch(thd, want_parts=True)
+            torch.cuda.synchronize()
+            total = parts.clone() if total is None else total + parts
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        full_lnl, full_parts = ctx.lnl_batch(thd, want_parts=True)
+        torch.cuda.synchronize()
+    ref = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th, cfg.spin_order)
+    assert_lnl_close(lnl_from_parts(total).cpu().numpy(), total.cpu().numpy(), ref[0], ref[1])
+    assert_lnl_close(full_lnl.cpu().numpy(), full_parts.cpu().numpy(), ref[0], ref[1])
