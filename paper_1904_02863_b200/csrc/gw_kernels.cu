@@ -210,15 +210,15 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
         const double pref = 3.0 / (128.0 * eta) / kTwoPi;
         const double kc2  = kc * kc;
         const double ik2  = ikap * ikap;
-        r[0 * S] = (3.0 / 128.0 / kTwoPi) / (kc2 * kc2 * kc);                       // c0  * x^-5
-        r[1 * S] = pref * phi2 * ik2 * ikap;                                        // c2  * x^-3
-        r[2 * S] = pref * phi3 * ik2;                                               // c3  * x^-2
-        r[3 * S] = pref * phi4 * ikap;                                              // c4  * x^-1
-        r[4 * S] = pref * (phi5 + ph5l * lnk) - (phic + 0.25 * kPi) / kTwoPi;       // c5  (constant)
-        r[5 * S] = pref * ph5l / 3.0;                                               // cL5 * ln f
-        r[6 * S] = pref * kap * (phi6 + ph6l * lnk);                                // c6  * x
-        r[7 * S] = pref * kap * ph6l / 3.0;                                         // cL6 * x ln f
-        r[8 * S] = pref * kap * kap * phi7;                                         // c7  * x^2
+        r[0 * S] = kPhaseScale * ((3.0 / 128.0 / kTwoPi) / (kc2 * kc2 * kc));                       // c0  * x^-5
+        r[1 * S] = kPhaseScale * (pref * phi2 * ik2 * ikap);                                        // c2  * x^-3
+        r[2 * S] = kPhaseScale * (pref * phi3 * ik2);                                               // c3  * x^-2
+        r[3 * S] = kPhaseScale * (pref * phi4 * ikap);                                              // c4  * x^-1
+        r[4 * S] = kPhaseScale * (pref * (phi5 + ph5l * lnk) - (phic + 0.25 * kPi) / kTwoPi);       // c5  (constant)
+        r[5 * S] = kPhaseScale * (pref * ph5l / 3.0);                                               // cL5 * ln f
+        r[6 * S] = kPhaseScale * (pref * kap * (phi6 + ph6l * lnk));                                // c6  * x
+        r[7 * S] = kPhaseScale * (pref * kap * ph6l / 3.0);                                         // cL6 * x ln f
+        r[8 * S] = kPhaseScale * (pref * kap * kap * phi7);                                         // c7  * x^2
         // NEXT-1 option isco_cut: f_ISCO = 1/(6^(3/2) pi M) and the last bin with f_j <= f_ISCO (-1: none).
         // The decision is taken in fp64 against the same f_j the oracle compares with.
         const double f_isco = 1.0 / (6.0 * sqrt(6.0) * (kap * kap * kap));         // kappa^3 = pi M
@@ -284,7 +284,7 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
         double rc_, rs_;
         cis_turns_of_product(-a.rot_stride_hz, tau, rc_, rs_);
         double *ri = r + (int64_t)(9 + kRecPerDet * i) * S;
-        ri[0 * S] = tau;
+        ri[0 * S] = kPhaseScale * tau;                       // in phase units (exact scaling)
         ri[1 * S] = a0 * (fp * pol_plus);                    // Re(A0 C_I),  C_I = F+ (1+cos^2 i)/2 - i Fx cos i
         ri[2 * S] = a0 * (-fc * cosi);                       // Im(A0 C_I)
         ri[3 * S] = rc_;
@@ -417,7 +417,7 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
 #pragma unroll
             for (int u = 0; u < kWfBins; ++u) {
                 double c, s;
-                cis_turns(__fma_rn(f[u], t_.x, ph[u]), c, s);
+                cis_phase(__fma_rn(f[u], t_.x, ph[u]), c, s);
                 const double kr = ca.x * amp[u], ki = ca.y * amp[u];
                 // (kr + i ki)(c - i s)
                 double2 out = make_double2(__fma_rn(kr, c, ki * s), __fma_rn(ki, c, -(kr * s)));
@@ -637,7 +637,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                     for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(tau[0], v[u].x, ph[u]);   // + f tau_0
                 }
 #pragma unroll
-                for (int u = 0; u < kUnroll; ++u) cis_turns(ph[u], cs[u], sn[u]);
+                for (int u = 0; u < kUnroll; ++u) cis_phase(ph[u], cs[u], sn[u]);
                 if (ISCO) {                                      // h = 0 above f_ISCO: the bin contributes nothing
 #pragma unroll
                     for (int u = 0; u < kUnroll; ++u)
@@ -674,7 +674,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                                     P[2 * kStageBins + jj], P[3 * kStageBins + jj]);
             ph = __fma_rn(tau[0], P[4 * kStageBins + jj].x, ph);
             double c, sn;
-            cis_turns(ph, c, sn);
+            cis_phase(ph, c, sn);
             if (ISCO && jstage + jj > jcut) { c = 0.0; sn = 0.0; }
 #pragma unroll
             for (int i = 0; i < NDET; ++i) {
@@ -705,7 +705,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
 #pragma unroll
         for (int i = 1; i < NDET; ++i) {
             double c, sn;
-            cis_turns_of_product(f_last, tau[i], c, sn);
+            cis_turns_of_product(f_last, tau[i] * (1.0 / kPhaseScale), c, sn);
             const double nr = __fma_rn(zr[i], c, -(zi[i] * sn));
             const double ni = __fma_rn(zr[i], sn, zi[i] * c);
             zr[i] = nr; zi[i] = ni;
