@@ -150,13 +150,14 @@ def run_reference(args):
     th = inputs.proposals(cfg)[:batch] if batch <= cfg.batch else inputs.proposals(cfg)
     # size one step to ~ (90 s budget) / (steps + warmup)
     per_step_s = min(10.0, 90.0 / max(1, args.steps + args.warmup))
-    rate, used, n, _, _ = oracle_rate(cfg, f, S, dets, d, th, min(per_step_s, 3.0))
+    cores = os.cpu_count() or 1          # torchrun exports OMP_NUM_THREADS=1; the oracle is timed on all host cores
+    rate, used, n, _, _ = oracle_rate(cfg, f, S, dets, d, th, min(per_step_s, 3.0), n_threads=cores)
     n = max(1, min(len(th), int(rate * per_step_s)))
     for _ in range(args.warmup):
-        oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order)
+        oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order, cores)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        _, _, used = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order)
+        _, _, used = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order, cores)
     dt = time.perf_counter() - t0
     value = n * args.steps / dt
     sample = f"first {n} of {batch} proposals of {name} per step, all {cfg.n_bins} bins x {cfg.n_det} detectors"
@@ -350,7 +351,7 @@ def run_ours(args):
     # ---- CPU baseline: the oracle as it stands on this box's host cores (rank 0, N = 1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        rate, used, n, dt, passes = oracle_rate(cfg, f, S, dets, d, th, args.cpu_seconds)
+        rate, used, n, dt, passes = oracle_rate(cfg, f, S, dets, d, th, args.cpu_seconds, n_threads=os.cpu_count() or 1)
         cpu = {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle",
                "sample": f"first {n} of {B} proposals x {passes} passes, all {M} bins x {n_det} detectors, {dt:.1f} s wall"}
         r1, u1, n1, dt1, p1 = oracle_rate(cfg, f, S, dets, d, th, min(3.0, args.cpu_seconds), n_threads=1)
