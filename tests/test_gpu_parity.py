@@ -292,3 +292,68 @@ def test_time_shift_interchange(oracle, torch_cuda):
     scale = np.abs(hb).max(axis=-1, keepdims=True)
     assert (np.abs(ha - hb) / scale).max() < 1e-11
     np.testing.assert_allclose(np.abs(ha), np.abs(hb), rtol=1e-12)
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_shapes(oracle, torch_cuda, seed):
+    """Seeded random shapes: bins 2..2500, proposals 1..700, 1..4 detectors (geometric and fixed mixed), random band,
+    resolution, mass range and options -- ragged tails everywhere the launch planner can put one."""
+    torch = torch_cuda
+    from paper_1904_02863_b200 import GwContext
+    rng = np.random.Generator(np.random.PCG64(4242 + seed))
+    n_det = int(rng.integers(1, 5))
+    M = int(rng.choice([2, 3, 5, 31, 33, 127, 129, 257, 640, 1000, 2500]))
+    B = int(rng.choice([1, 2, 5, 8, 17, 32, 100, 255, 256, 300, 700]))
+    df = float(rng.choice([1 / 128, 1 / 16, 0.125, 0.25, 1.0]))
+    f0 = float(rng.choice([10.0, 20.0, 35.5]))
+    f = f0 + np.arange(M) * df
+    bns = bool(rng.integers(0, 2))
+    isco, marg, spin = int(rng.integers(0, 2)), int(rng.integers(0, 2)), int(rng.integers(0, 2))
+    names = ["H1", "L1", "V1"]
+    rows = []
+    for i in range(n_det):
+        if rng.random() < 0.3:
+            rows.append(inputs.fixed_detector(float(rng.uniform(-1, 1)), float(rng.uniform(-1, 1)), float(rng.uniform(-0.03, 0.03))))
+        else:
+            rows.append(inputs.geometric_detector(names[int(rng.integers(0, 3))]))
+    dets = np.stack(rows)
+    S = np.stack([inputs.analytic_psd(f) * float(rng.uniform(0.5, 2.0)) for _ in range(n_det)])
+    th = np.empty((B, 11))
+    th[:, inputs.P_MC] = rng.uniform(1.0, 2.0, B) if bns else rng.uniform(5.0, 60.0, B)
+    th[:, inputs.P_Q] = rng.uniform(0.2, 1.0, B)
+    th[:, inputs.P_CHI1] = rng.uniform(-0.9, 0.9, B)
+    th[:, inputs.P_CHI2] = rng.uniform(-0.9, 0.9, B)
+    th[:, inputs.P_DL] = rng.uniform(50, 3000, B)
+    th[:, inputs.P_TC] = rng.uniform(-0.5, 0.5, B)
+    th[:, inputs.P_PHIC] = rng.uniform(-7, 7, B)
+    th[:, inputs.P_COSI] = rng.uniform(-1, 1, B)
+    th[:, inputs.P_RA] = rng.uniform(0, 2 * np.pi, B)
+    th[:, inputs.P_DEC] = np.arcsin(rng.uniform(-1, 1, B))
+    th[:, inputs.P_PSI] = rng.uniform(0, np.pi, B)
+    gmst = float(rng.uniform(0, 2 * np.pi))
+    z = rng.standard_normal((n_det, M, 2))
+    d = oracle.waveform(f, dets, gmst, th[:1], spin)[0] + (z[..., 0] + 1j * z[..., 1]) * np.sqrt(S / (4 * df))
+    with GwContext(f, d, S, dets, gmst, spin_order=spin, max_batch=B, isco_cut=isco, phase_marginal=marg) as ctx:
+        thd = _dev(torch, th)
+        lnl, parts = ctx.lnl_batch(thd, want_parts=True)
+        h = ctx.waveform_batch(thd[: min(B, 16)].contiguous())
+        torch.cuda.synchronize()
+        lnl, parts, h = lnl.cpu().numpy(), parts.cpu().numpy(), h.cpu().numpy()
+    lnl_ref, parts_ref, _ = oracle.lnl(f, df, d, S, dets, gmst, th, spin, isco_cut=isco)
+    if marg:
+        lnl_ref = oracle.lnl_phase_marginal(parts_ref)
+    hh = parts_ref[..., 2].sum(axis=1)
+    keep = hh > 0                                     # isco_cut below the band: h = 0, lnL = 0 exactly
+    assert np.all(lnl[~keep] == 0) and np.all(parts[~keep] == 0)
+    if keep.any():
+        scale = np.abs(parts_ref[keep][..., 0].sum(axis=1)) + hh[keep]
+        assert (np.abs(lnl[keep] - lnl_ref[keep]) / scale).max() <= 1e-8
+        pscale = (np.hypot(parts_ref[keep][..., 0], parts_ref[keep][..., 1]) + parts_ref[keep][..., 2])[..., None]
+        ok = pscale[..., 0] > 0
+        assert (np.abs(parts[keep] - parts_ref[keep])[ok] / pscale[ok]).max() <= 1e-8
+    h_ref = oracle.waveform(f, dets, gmst, th[: min(B, 16)], spin, isco_cut=isco)
+    hs = np.abs(h_ref).max(axis=-1, keepdims=True)
+    nz = hs[..., 0] > 0
+    assert np.all(h[~nz] == 0)
+    if nz.any():
+        assert (np.abs(h - h_ref)[nz] / hs[nz]).max() <= 1e-9
