@@ -357,3 +357,37 @@ def test_random_shapes(oracle, torch_cuda, seed):
     assert np.all(h[~nz] == 0)
     if nz.any():
         assert (np.abs(h - h_ref)[nz] / hs[nz]).max() <= 1e-9
+
+
+def test_cuda_phase_against_40_digit_arithmetic(torch_cuda):
+    """Pin P7 applied to the CUDA path itself (no oracle involved): arg h of a FIXED (F+ = 1, Fx = 0, dt = 0) detector
+    against the 40-digit TaylorF2 phase of tests/test_oracle_phase.py, to the same ulp-relative bound as the oracle."""
+    torch = torch_cuda
+    import mpmath as mp
+    from test_oracle_phase import _mp_phase
+    from paper_1904_02863_b200 import GwContext
+    mp.mp.dps = 40
+    rng = np.random.default_rng(11)
+    f = np.array([10.0, 10.0 + 1 / 512, 13.7, 20.0, 33.25, 64.0, 150.5, 512.0, 1024.0, 2047.5])
+    f = 10.0 + np.round((f - 10.0) * 512) / 512                       # on a uniform 1/512 Hz grid
+    grid = 10.0 + np.arange(int(round((f.max() - 10.0) * 512)) + 1) / 512
+    idx = np.round((f - 10.0) * 512).astype(int)
+    th = np.zeros((24, 11))
+    for b in range(24):
+        bns = b % 2 == 0
+        th[b] = [rng.uniform(1.1, 1.3) if bns else rng.uniform(20, 40), rng.uniform(0.5, 1), rng.uniform(-0.8, 0.8),
+                 rng.uniform(-0.8, 0.8), 100.0, rng.uniform(-0.1, 0.1), rng.uniform(0, 2 * np.pi), 1.0, 0, 0, 0]
+    S = np.ones((1, grid.size))
+    d = np.zeros((1, grid.size), complex)
+    with GwContext(grid, d, S, inputs.fixed_detector(1.0, 0.0, 0.0)[None], 0.0, max_batch=24) as ctx:
+        h = ctx.waveform_batch(_dev(torch, th))[:, 0, :][:, _dev(torch, idx)].cpu().numpy()
+    worst = 0.0
+    for b in range(24):
+        for k, fk in enumerate(grid[idx]):
+            want = _mp_phase(fk, th[b], 1, None)
+            got = np.angle(h[b, k])                                    # arg h = -Psi (mod 2 pi)
+            err = float(abs(mp.mpf(got) + want - 2 * mp.pi * mp.nint((mp.mpf(got) + want) / (2 * mp.pi))))
+            bound = 16 * np.spacing(float(abs(want))) + 1e-13
+            worst = max(worst, err / bound)
+            assert err < bound, (b, fk, err, bound)
+    assert worst > 0
