@@ -34,7 +34,8 @@
  *     outputs (fixed-order reductions only; no floating-point atomics).
  *   - theta lives on the device and is not validated on the host.  A proposal with Mc <= 0, q outside
  *     (0, 1], D <= 0, |cos iota| > 1, |chi| > 1 or any non-finite entry yields NaN in that proposal's
- *     outputs and does not affect other proposals.
+ *     outputs and does not affect other proposals.  So does a proposal whose phase could exceed 2.5e8 turns
+ *     anywhere in the band (e.g. Mc < ~2e-3 Msun from 10 Hz), the domain of the integer range reduction.
  *   - All arithmetic is IEEE fp64; complex numbers are interleaved (re, im) pairs of doubles.
  */
 #ifndef GWLNL_H

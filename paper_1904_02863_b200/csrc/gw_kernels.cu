@@ -156,7 +156,7 @@ struct SetupArgs {
     int     relative_tau;     // 1: tau_I (I >= 1) and rot_I are relative to detector 0 (fused kernel); 0: absolute
     const double2 *f_amp;     // basis plane 4: (f_j, f_j^-7/6), for the f_ISCO bin search
     int64_t n_bins;
-    double  f0, delta_f;
+    double  f0, delta_f, f_max;
 };
 
 // A CTA of 128 threads serves 32 proposals; warp w takes role w for proposal (block*32 + lane), so the four
@@ -219,6 +219,16 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
         r[6 * S] = kPhaseScale * (pref * kap * (phi6 + ph6l * lnk));                                // c6  * x
         r[7 * S] = kPhaseScale * (pref * kap * ph6l / 3.0);                                         // cL6 * x ln f
         r[8 * S] = kPhaseScale * (pref * kap * kap * phi7);                                         // c7  * x^2
+        {   // domain of the integer range reduction (cis_quarter_turns: |phase| < 2^31 quarter turns): bound the
+            // phase over the band by its terms at the band edges; beyond 1e9 phase units the proposal is poisoned
+            const double x0 = cbrt(a.f0), xi = 1.0 / x0, x1 = cbrt(a.f_max), tc = th[GW_P_TC];
+            const double l1 = fmax(fabs(log(a.f0)), fabs(log(a.f_max)));
+            const double bound = fabs(r[0 * S]) * (xi * xi) * (xi * xi) * xi + fabs(r[1 * S]) * (xi * xi * xi) +
+                                 fabs(r[2 * S]) * (xi * xi) + fabs(r[3 * S]) * xi + fabs(r[4 * S]) +
+                                 fabs(r[5 * S]) * l1 + fabs(r[6 * S]) * x1 + fabs(r[7 * S]) * x1 * l1 +
+                                 fabs(r[8 * S]) * x1 * x1 + kPhaseScale * (fabs(tc) + 1.0) * a.f_max;
+            if (!(bound < 1.0e9)) r[4 * S] = __longlong_as_double(0x7ff8000000000000LL);
+        }
         // NEXT-1 option isco_cut: f_ISCO = 1/(6^(3/2) pi M) and the last bin with f_j <= f_ISCO (-1: none).
         // The decision is taken in fp64 against the same f_j the oracle compares with.
         const double f_isco = 1.0 / (6.0 * sqrt(6.0) * (kap * kap * kap));         // kappa^3 = pi M
@@ -302,6 +312,7 @@ cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int s
     a.rot_stride_hz = rot_stride_hz; a.relative_tau = relative_tau;
     a.f_amp = reinterpret_cast<const double2 *>(t.planes) + 4 * t.n_pad;
     a.n_bins = t.n_bins; a.f0 = t.f0; a.delta_f = t.delta_f;
+    a.f_max = t.f0 + (double)(t.n_bins - 1) * t.delta_f;
     const unsigned blocks = (unsigned)((n_prop + 31) / 32);
     setup_kernel<<<blocks, 128, 0, s>>>(a);
     *launches += 1;

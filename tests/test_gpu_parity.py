@@ -391,3 +391,26 @@ def test_cuda_phase_against_40_digit_arithmetic(torch_cuda):
             worst = max(worst, err / bound)
             assert err < bound, (b, fk, err, bound)
     assert worst > 0
+
+
+def test_phase_domain_guard(oracle, torch_cuda):
+    """A proposal whose phase would leave the domain of the integer range reduction (|phase| >= 2^31 quarter turns)
+    gives NaN, not garbage; one well inside the domain (Mc = 0.05 Msun, 3.6e6 turns at 10 Hz) still matches the oracle."""
+    torch = torch_cuda
+    from paper_1904_02863_b200 import GwContext
+    f = 10.0 + np.arange(400) / 16.0
+    S = inputs.analytic_psd(f)[None]
+    dets = inputs.fixed_detector(1.0, 0.0, 0.0)[None]
+    th = np.tile(np.array(inputs.CONFIGS["C0"].theta_inj), (3, 1))
+    th[0, inputs.P_MC] = 0.05
+    th[1, inputs.P_MC] = 1.0e-4          # ~1e11 turns at 10 Hz: out of domain
+    rng = np.random.Generator(np.random.PCG64(5))
+    d = (rng.standard_normal((1, f.size)) + 1j * rng.standard_normal((1, f.size))) * np.sqrt(S / (4 / 16.0))
+    with GwContext(f, d, S, dets, 0.0, spin_order=0, max_batch=3) as ctx:
+        lnl, parts = ctx.lnl_batch(_dev(torch, th), want_parts=True)
+        h = ctx.waveform_batch(_dev(torch, th))
+        torch.cuda.synchronize()
+        lnl, parts, h = lnl.cpu().numpy(), parts.cpu().numpy(), h.cpu().numpy()
+    assert np.isnan(lnl[1]) and np.all(np.isnan(h[1])) and np.all(np.isfinite(lnl[[0, 2]]))
+    ref = oracle.lnl(f, 1 / 16.0, d, S, dets, 0.0, th[[0, 2]], 0)
+    assert_lnl_close(lnl[[0, 2]], parts[[0, 2]], ref[0], ref[1])
