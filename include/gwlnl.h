@@ -30,6 +30,8 @@
  *     host and device (the paper's reusable-buffer lesson).  The *_host variants
  *     copy in, compute, copy out and synchronise the stream before returning.
  *   - A context may be used from one stream at a time (it owns one workspace).
+ *   - A context belongs to the device that was current in gw_ctx_create; later calls make that device current
+ *     for their duration and restore the caller's.
  *   - Determinism: same context, same theta, same n_prop, same build, same GPU model => bit-identical
  *     outputs (fixed-order reductions only; no floating-point atomics).
  *   - theta lives on the device and is not validated on the host.  A proposal with Mc <= 0, q outside

@@ -154,6 +154,19 @@ int reserve_impl(gw_ctx *ctx, int64_t max_batch)
 
 bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
 
+// Makes the context's device current for the duration of a call and restores the caller's device afterwards
+// (a no-op when it is current already, which is the one-process-per-GPU case).
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const gw_ctx *ctx)
+    {
+        if (ctx && cudaGetDevice(&prev) == cudaSuccess && prev != ctx->device)
+            switched = cudaSetDevice(ctx->device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
 int check_batch_args(gw_ctx *ctx, int64_t n_prop, const void *theta, const void *out)
 {
     if (!ctx || n_prop < 0) return GW_ERR_INVALID_ARG;
@@ -297,12 +310,14 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
 int gw_ctx_reserve(gw_ctx *ctx, int64_t max_batch)
 {
     if (!ctx || max_batch < 1) return GW_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx);
     return reserve_impl(ctx, max_batch);
 }
 
 int gw_ctx_destroy(gw_ctx *ctx)
 {
     if (!ctx) return GW_OK;
+    DeviceGuard guard(ctx);
     cudaDeviceSynchronize();
     free_workspace(ctx->w);
     cudaFree(ctx->t.planes); cudaFree(ctx->t.i7cum);
@@ -374,6 +389,7 @@ int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *l
 {
     int rc = check_batch_args(ctx, n_prop, theta_dev, lnl_out_dev);
     if (rc != GW_OK || n_prop == 0) return rc;
+    DeviceGuard guard(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Plan p = make_plan(ctx, n_prop);
     if (partial_need(ctx, p) > ctx->w.partial_doubles || p.n_tiles > ctx->w.n_tickets) return GW_ERR_INVALID_ARG;
@@ -394,6 +410,7 @@ int gw_waveform_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, doub
     int rc = check_batch_args(ctx, n_prop, theta_dev, h_out_dev);
     if (rc != GW_OK || n_prop == 0) return rc;
     if (((uintptr_t)h_out_dev & 15u) != 0) return GW_ERR_INVALID_ARG;
+    DeviceGuard guard(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     if (ctx->timing) cudaEventRecord(ctx->ev[0], s);
     cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
@@ -411,6 +428,7 @@ int gw_lnl_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, dou
 {
     int rc = check_batch_args(ctx, n_prop, theta_host, lnl_out_host);
     if (rc != GW_OK || n_prop == 0) return rc;
+    DeviceGuard guard(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     Workspace &w = ctx->w;
     cudaError_t e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * GW_NPARAM,
@@ -432,6 +450,7 @@ int gw_waveform_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host
 {
     int rc = check_batch_args(ctx, n_prop, theta_host, h_out_host);
     if (rc != GW_OK || n_prop == 0) return rc;
+    DeviceGuard guard(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     Workspace &w = ctx->w;
     const int64_t per_prop = (int64_t)ctx->t.n_det * ctx->t.n_bins * 2;
