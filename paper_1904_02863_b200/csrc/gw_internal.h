@@ -18,6 +18,9 @@ namespace gw {
 #ifndef GW_UNROLL
 #define GW_UNROLL 4
 #endif
+#ifndef GW_PIPELINE
+#define GW_PIPELINE 1
+#endif
 #ifndef GW_STAGE_BINS
 #define GW_STAGE_BINS 128
 #endif

@@ -614,8 +614,9 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             // share a register operand in the same slot (the coefficient across bins, c/s across detectors,
             // z across the re/im pair), which the operand-reuse cache serves.  A DFMA with three fresh
             // register operands issues at 2/3 rate on B200 (profiles/dfma_operand_probe).
-            for (; it + kUnroll <= iters; it += kUnroll) {
-                double ph[kUnroll], cs[kUnroll], sn[kUnroll];
+            // E(it0): phase and sincos of kUnroll bins; U(it0): their detector updates (ascending bin order).
+            auto compute_e = [&](int it, double (&cs)[kUnroll], double (&sn)[kUnroll]) {
+                double ph[kUnroll];
                 {
                     double2 v[kUnroll];
 #pragma unroll
@@ -654,6 +655,8 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                     for (int u = 0; u < kUnroll; ++u)
                         if (jstage + it + u > jcut) { cs[u] = 0.0; sn[u] = 0.0; }
                 }
+            };
+            auto update_z = [&](int it, const double (&cs)[kUnroll], const double (&sn)[kUnroll]) {
 #pragma unroll
                 for (int u = 0; u < kUnroll; ++u) {              // bins in ascending order: the Z recurrence
 #pragma unroll
@@ -675,7 +678,30 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                         zr[i] = nr; zi[i] = ni;
                     }
                 }
+            };
+#if GW_PIPELINE
+            // software pipeline: the sincos of the next kUnroll bins is issued together with the detector
+            // updates of the current ones (two independent instruction streams in one basic block)
+            if (iters >= kUnroll) {
+                double cs[kUnroll], sn[kUnroll];
+                compute_e(0, cs, sn);
+                for (; it + 2 * kUnroll <= iters; it += kUnroll) {
+                    double cn[kUnroll], sm_[kUnroll];
+                    compute_e(it + kUnroll, cn, sm_);
+                    update_z(it, cs, sn);
+#pragma unroll
+                    for (int u = 0; u < kUnroll; ++u) { cs[u] = cn[u]; sn[u] = sm_[u]; }
+                }
+                update_z(it, cs, sn);
+                it += kUnroll;
             }
+#else
+            for (; it + kUnroll <= iters; it += kUnroll) {
+                double cs[kUnroll], sn[kUnroll];
+                compute_e(it, cs, sn);
+                update_z(it, cs, sn);
+            }
+#endif
         }
         for (; it < iters; ++it) {
             int jj = MULTI ? sub + it * lpp : it;
