@@ -16,13 +16,13 @@ namespace gw {
 #define GW_MIN_CTAS 2
 #endif
 #ifndef GW_UNROLL
-#define GW_UNROLL 4
+#define GW_UNROLL 5
 #endif
 #ifndef GW_PIPELINE
 #define GW_PIPELINE 1
 #endif
 #ifndef GW_STAGE_BINS
-#define GW_STAGE_BINS 128
+#define GW_STAGE_BINS 160
 #endif
 #ifndef GW_STAGES
 #define GW_STAGES 3
