@@ -5,7 +5,7 @@
 //   K2 waveform_kernel                 : complex128 h(f) to HBM                 (DESIGN.md 6.K2; a6)
 //   K3 fused_kernel                    : phase + projection + <d|h>, fixed-order finish (6.K3; a2..a5)
 //
-// Phase convention: everything is carried in TURNS.  With x = f^(1/3), L = ln f
+// Phase convention: everything is carried in units of 1/kPhaseScale turns (quarter turns).  With x = f^(1/3), L = ln f
 // and the per-bin basis b = (x^-5, x^-3, x^-2, x^-1, L, x, xL, x^2),
 //     Phi'(f) = c5 + c0 b0 + c2 b1 + c3 b2 + c4 b3 + cL5 b4 + c6 b5 + cL6 b6 + c7 b7          [turns]
 // is the TaylorF2 phase WITHOUT the 2 pi f t_c term; t_c is merged with the detector delay,
@@ -482,7 +482,7 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
 // chunk; the tables are read from shared memory as warp broadcasts), 2..32 for small batches (the lanes
 // of a proposal interleave over the bins; a fixed xor-shuffle tree combines them).
 // The chunk is streamed through a kStages-deep ring of kStageBins-bin stages by bulk async copies (TMA
-// engine) completing on mbarriers.  Per (proposal, bin): 9 FMA phase (incl. f tau_0), 16-op sincos giving
+// engine) completing on mbarriers.  Per (proposal, bin): 9 FMA phase (incl. f tau_0), 14-op sincos (cis_phase) giving
 // E = e^{+2 pi i (Phi' + f tau_0)}, detector 0: Z_0 += g_0j E (4 FMA), and per detector I >= 1
 //     Z_I <- Z_I * rot_I + g_Ij * E                                                  (8 fp64 ops)
 // where rot_I = exp(-2 pi i lpp df (tau_I - tau_0)): after the sweep Z_I * exp(+2 pi i f_last (tau_I - tau_0))
