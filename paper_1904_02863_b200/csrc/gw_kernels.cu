@@ -703,6 +703,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             }
 #endif
         }
+#pragma unroll (MULTI ? 4 : 1)
         for (; it < iters; ++it) {
             int jj = MULTI ? sub + it * lpp : it;
             bool masked = false;
