@@ -779,6 +779,35 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
     if (s_ticket != (unsigned)(a.n_chunks - 1)) return;
     // stage 2 (last CTA of the tile): chunks summed in index order
     __threadfence();
+    {   // Small tiles (multi-lane layouts): all threads pull the tile's partials into the now idle stage buffers in
+        // one round trip to L2, and the ordered sums read shared memory.  Same additions in the same order as the
+        // direct path below, so the bits do not depend on which path runs.
+        const int nvals = PT * 2 * NDET * a.n_chunks;
+        if (MULTI && nvals <= kStages * NP * kStageBins * 2) {
+            double *sh = reinterpret_cast<double *>(smem_raw);
+            const double *src = a.partial + (tile * a.n_chunks * (int64_t)(2 * NDET)) * PT;
+            for (int i = tid; i < nvals; i += kThreads) sh[i] = __ldcg(src + i);
+            __syncthreads();
+            if (tid < PT) {
+                const int64_t bb = tile * PT + tid;
+                if (bb < a.n_prop) {
+                    double sr[NDET], si[NDET];
+#pragma unroll
+                    for (int i = 0; i < NDET; ++i) { sr[i] = 0.0; si[i] = 0.0; }
+                    for (int c = 0; c < a.n_chunks; ++c) {
+#pragma unroll
+                        for (int i = 0; i < NDET; ++i) {
+                            sr[i] += sh[(c * 2 * NDET + 2 * i) * PT + tid];
+                            si[i] += sh[(c * 2 * NDET + 2 * i + 1) * PT + tid];
+                        }
+                    }
+                    finish_proposal<NDET, ISCO>(a, bb, sr, si);
+                }
+            }
+            if (tid == 0) a.tickets[tile] = 0u;
+            return;
+        }
+    }
     if (tid < PT) {
         const int64_t bb = tile * PT + tid;
         if (bb < a.n_prop) {
