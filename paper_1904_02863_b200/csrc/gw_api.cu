@@ -52,7 +52,10 @@ constexpr double kProBins  = 14.0;
 constexpr double kSatWarps = 3.0;
 constexpr int    kMaxChunks = 4096;
 constexpr int64_t kMaxWaves = 8;
-constexpr double kMultiPenalty = 1.35;     // the lanes-interleaved loop costs this much more per bin (measured, C2)
+#ifndef GW_MULTI_PENALTY
+#define GW_MULTI_PENALTY 1.35
+#endif
+constexpr double kMultiPenalty = GW_MULTI_PENALTY;     // the lanes-interleaved loop costs this much more per bin (measured, C2)
 constexpr double kFinishPerChunk = 0.25;   // last-CTA cross-chunk sum, in bin-sweep equivalents per chunk
 
 Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
