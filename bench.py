@@ -276,8 +276,9 @@ def run_ours(args):
     peak = n_sm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     roofline = {"bound": "alu", "kernel": "fused_kernel<%d>" % n_det, "achieved": achieved, "peak": peak,
                 "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(name) if B == cfg.batch else None,
-                "peak_source": "derived: %d SMs x %d fp64 FMA lanes x 2 flop x %.0f MHz (MEASURED_PEAKS sm_max_mhz)"
-                               % (n_sm, FP64_LANES_PER_SM, sm_max),
+                "peak_source": "derived: %d SMs x %d fp64 FMA lanes x 2 flop x %.0f MHz (%s)"
+                               % (n_sm, FP64_LANES_PER_SM, sm_max,
+                                  "MEASURED_PEAKS.json sm_max_mhz" if "sm_max_mhz" in peaks else "fallback clock, B200_PROFILING.md"),
                 "peak_measured_fma_probe": 2 * fma_rate / 1e12, "frac_of_measured": achieved / (2 * fma_rate / 1e12),
                 "flop_per_launch": flops_per_launch, "walg_fma_per_prop_bin": walg,
                 "kernel_ms": fused_ms, "setup_kernel_ms": float(np.mean(s_ms))}
@@ -344,7 +345,7 @@ def run_ours(args):
         hbm = float(peaks.get("hbm_gbs", 6650.0))
         extra["waveform_kernel"] = {"proposals": wb, "bytes_stored": wb * n_det * M * 16, "kernel_ms": float(np.mean(w_ms)),
                                     "achieved_GBps": gbs, "hbm_peak_GBps": hbm,
-                                    "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback",
+                                    "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)",
                                     "frac": gbs / hbm}
         del h
 
