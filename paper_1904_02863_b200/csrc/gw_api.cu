@@ -64,7 +64,7 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
     const int slots_per_sm = ctx->ctas_per_sm > 0 ? ctx->ctas_per_sm : 1;
     const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 148;
     const int64_t slots = (int64_t)n_sm * slots_per_sm;
-    Plan best = {1, kThreads, 1, (n_prop + kThreads - 1) / kThreads};
+    Plan best = {1, kThreads, 1, (n_prop + kThreads - 1) / kThreads, 1};
     double best_cost = 1e300;
     for (int lpp = 1; lpp <= 32; lpp *= 2) {
         const int pt = kThreads / lpp;
@@ -92,6 +92,7 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
         }
         if (tiles >= slots) break;                            // enough proposals to fill the GPU: keep this lpp
     }
+    best.n_groups = best.n_chunks >= kFinishTwoLevelFrom ? (best.n_chunks + kFinishGroup - 1) / kFinishGroup : 1;
     return best;
 }
 
@@ -111,7 +112,8 @@ int64_t partial_need(const gw_ctx *ctx, const Plan &p)
 
 void free_workspace(Workspace &w)
 {
-    cudaFree(w.rec); cudaFree(w.partial); cudaFree(w.tickets); cudaFree(w.theta_stage);
+    cudaFree(w.rec); cudaFree(w.partial); cudaFree(w.tickets); cudaFree(w.gpartial); cudaFree(w.gtickets);
+    cudaFree(w.theta_stage);
     cudaFree(w.lnl_stage); cudaFree(w.parts_stage); cudaFree(w.h_stage);
     std::memset(&w, 0, sizeof(w));
 }
@@ -131,11 +133,17 @@ int reserve_impl(gw_ctx *ctx, int64_t max_batch)
     const int64_t n_rec = rec_fields(n_det);
     w.partial_doubles = need_partial > 0 ? need_partial : 1;
     w.n_tickets = need_tickets;
+    // two-level finish: n_groups <= n_chunks / 8 whenever it is used (n_chunks >= 33, groups of 16)
+    w.gpartial_doubles = w.partial_doubles / 8 + 1;
+    w.n_gtickets = need_partial / ((int64_t)kThreads * 2 * n_det) / 8 + need_tickets + 1;
     w.h_stage_doubles = 0;                                    // the host waveform variant allocates its slab on first use
     bool ok = true;
     ok = ok && (e = cudaMalloc(&w.rec, sizeof(double) * n_rec * w.rec_stride)) == cudaSuccess;
     ok = ok && (e = cudaMalloc(&w.partial, sizeof(double) * w.partial_doubles)) == cudaSuccess;
     ok = ok && (e = cudaMalloc(&w.tickets, sizeof(unsigned int) * w.n_tickets)) == cudaSuccess;
+    ok = ok && (e = cudaMalloc(&w.gpartial, sizeof(double) * w.gpartial_doubles)) == cudaSuccess;
+    ok = ok && (e = cudaMalloc(&w.gtickets, sizeof(unsigned int) * w.n_gtickets)) == cudaSuccess;
+    ok = ok && (e = cudaMemset(w.gtickets, 0, sizeof(unsigned int) * w.n_gtickets)) == cudaSuccess;
     ok = ok && (e = cudaMalloc(&w.theta_stage, sizeof(double) * max_batch * GW_NPARAM)) == cudaSuccess;
     ok = ok && (e = cudaMalloc(&w.lnl_stage, sizeof(double) * max_batch)) == cudaSuccess;
     ok = ok && (e = cudaMalloc(&w.parts_stage, sizeof(double) * max_batch * n_det * 3)) == cudaSuccess;
@@ -396,12 +404,15 @@ int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *l
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Plan p = make_plan(ctx, n_prop);
     if (partial_need(ctx, p) > ctx->w.partial_doubles || p.n_tiles > ctx->w.n_tickets) return GW_ERR_INVALID_ARG;
+    if (p.n_groups > 1 && (p.n_tiles * p.n_groups * (int64_t)(2 * ctx->t.n_det) * p.props_per_cta > ctx->w.gpartial_doubles ||
+                           p.n_tiles * p.n_groups > ctx->w.n_gtickets))
+        return GW_ERR_INVALID_ARG;
     if (ctx->timing) cudaEventRecord(ctx->ev[0], s);
     cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
                                  ctx->w.rec_stride, (double)p.lpp * ctx->t.delta_f, 1, s, &ctx->launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     if (ctx->timing) cudaEventRecord(ctx->ev[1], s);
-    e = launch_fused(ctx->t, p, n_prop, ctx->w.rec, ctx->w.rec_stride, ctx->w.partial, ctx->w.tickets, lnl_out_dev,
+    e = launch_fused(ctx->t, p, n_prop, ctx->w.rec, ctx->w.rec_stride, ctx->w.partial, ctx->w.tickets, ctx->w.gpartial, ctx->w.gtickets, lnl_out_dev,
                      parts_out_dev, s, &ctx->launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     if (ctx->timing) cudaEventRecord(ctx->ev[2], s);

@@ -34,6 +34,8 @@ constexpr int kStages     = GW_STAGES;      // stage ring depth
 constexpr int kUnroll     = GW_UNROLL;      // bins per unrolled trip of the fused hot loop
 constexpr int kBasis      = 8;     // per-bin phase basis values (4 planes of 2)
 constexpr int kBasisPlanes = 5;    // (x^-5,x^-3) (x^-2,x^-1) (ln f,x) (x ln f,x^2) (f,f^-7/6)
+constexpr int kFinishGroup = 16;   // chunks per group of the two-level finish
+constexpr int kFinishTwoLevelFrom = 33;  // n_chunks from which the finish is two-level
 constexpr int kRecFixed   = 10;    // record fields before the per-detector block
 constexpr int kRecPerDet  = 5;     // tau, Cre, Cim, rot_re, rot_im
 // record fields: 0..8 phase coefficients, then kRecPerDet per detector, then f_ISCO and the index of the last
@@ -69,6 +71,7 @@ struct Plan {
     int     props_per_cta;// kThreads / lpp
     int     n_chunks;     // frequency chunks per proposal tile
     int64_t n_tiles;      // ceil(n_prop / props_per_cta)
+    int     n_groups;     // 1, or ceil(n_chunks / kFinishGroup) when the finish is two-level
 };
 
 struct Workspace {
@@ -79,6 +82,10 @@ struct Workspace {
     int64_t partial_doubles;
     unsigned int *tickets;// [max tiles]
     int64_t n_tickets;
+    double *gpartial;     // group sums of the two-level finish, gpartial_doubles
+    int64_t gpartial_doubles;
+    unsigned int *gtickets;
+    int64_t n_gtickets;
     double *theta_stage;  // [max_batch][GW_NPARAM]   (host-variant staging)
     double *lnl_stage;    // [max_batch]
     double *parts_stage;  // [max_batch][n_det][3]
@@ -93,8 +100,8 @@ cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int s
                          const double *theta_dev, double *rec, int64_t rec_stride, double rot_stride_hz,
                          int relative_tau, cudaStream_t s, int64_t *launches);
 cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, const double *rec,
-                         int64_t rec_stride, double *partial, unsigned int *tickets, double *lnl_out,
-                         double *parts_out, cudaStream_t s, int64_t *launches);
+                         int64_t rec_stride, double *partial, unsigned int *tickets, double *gpartial,
+                         unsigned int *gtickets, double *lnl_out, double *parts_out, cudaStream_t s, int64_t *launches);
 cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, int64_t rec_stride,
                             double *h_out, cudaStream_t s, int64_t *launches);
 cudaError_t configure_kernels(int *fused_ctas_per_sm);      // smem attributes + occupancy query (per n_det below)

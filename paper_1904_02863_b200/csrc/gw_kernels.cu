@@ -501,6 +501,9 @@ struct FusedArgs {
     int     phase_marginal;
     double *partial;
     unsigned int *tickets;
+    int     n_groups;        // > 1: two-level finish over groups of kFinishGroup chunks
+    double *gpartial;        // [tile][group][2 NDET][PT] group sums
+    unsigned int *gtickets;  // [tile][group]
     double *lnl, *parts;
 };
 
@@ -772,18 +775,71 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             part[(2 * i + 1) * PT + pic] = zi[i];
         }
     }
+    // Ordered sum of `count` entries (chunks or groups) of one proposal: entry e, component q at base[(e*2*NDET+q)*PT].
+    // Loads of kFinishBatch entries are issued together (the sum is latency-bound on L2 otherwise); the additions
+    // stay in index order, so the result does not depend on the batching.
+    auto ordered_sum = [&](const double *base, int count, double (&sr)[NDET], double (&si)[NDET]) {
+        constexpr int kFinishBatch = 8;
+        int c = 0;
+        for (; c + kFinishBatch <= count; c += kFinishBatch) {
+            double v[kFinishBatch][2 * NDET];
+#pragma unroll
+            for (int u = 0; u < kFinishBatch; ++u)
+#pragma unroll
+                for (int q = 0; q < 2 * NDET; ++q)
+                    v[u][q] = __ldcg(base + ((int64_t)(c + u) * 2 * NDET + q) * PT);
+#pragma unroll
+            for (int u = 0; u < kFinishBatch; ++u)
+#pragma unroll
+                for (int i = 0; i < NDET; ++i) { sr[i] += v[u][2 * i]; si[i] += v[u][2 * i + 1]; }
+        }
+        for (; c < count; ++c) {
+#pragma unroll
+            for (int i = 0; i < NDET; ++i) {
+                sr[i] += __ldcg(base + ((int64_t)c * 2 * NDET + 2 * i) * PT);
+                si[i] += __ldcg(base + ((int64_t)c * 2 * NDET + 2 * i + 1) * PT);
+            }
+        }
+    };
     __threadfence();
     __syncthreads();
+    unsigned int last_ticket = (unsigned)(a.n_chunks - 1);
+    if (a.n_groups > 1) {
+        // Two-level finish for many chunks (a single CTA summing hundreds of chunk partials is bound by one SM's L2
+        // bandwidth): the last CTA of each group of kFinishGroup chunks sums that group in chunk order, and the
+        // last group to finish sums the group sums in group order.  The order is fixed by (n_chunks, kFinishGroup).
+        const int group = chunk / kFinishGroup;
+        const int gsize = min(kFinishGroup, a.n_chunks - group * kFinishGroup);
+        unsigned int *gt = a.gtickets + tile * a.n_groups + group;
+        if (tid == 0) s_ticket = atomicAdd(gt, 1u);
+        __syncthreads();
+        if (s_ticket != (unsigned)(gsize - 1)) return;
+        __threadfence();
+        if (tid < PT) {
+            double sr[NDET], si[NDET];
+#pragma unroll
+            for (int i = 0; i < NDET; ++i) { sr[i] = 0.0; si[i] = 0.0; }
+            ordered_sum(a.partial + ((tile * a.n_chunks + (int64_t)group * kFinishGroup) * (int64_t)(2 * NDET)) * PT + tid,
+                        gsize, sr, si);
+            double *gp = a.gpartial + ((tile * a.n_groups + group) * (int64_t)(2 * NDET)) * PT + tid;
+#pragma unroll
+            for (int i = 0; i < NDET; ++i) { gp[(2 * i) * PT] = sr[i]; gp[(2 * i + 1) * PT] = si[i]; }
+        }
+        if (tid == 0) *gt = 0u;
+        __threadfence();
+        __syncthreads();
+        last_ticket = (unsigned)(a.n_groups - 1);
+    }
     if (tid == 0) s_ticket = atomicAdd(&a.tickets[tile], 1u);
     __syncthreads();
-    if (s_ticket != (unsigned)(a.n_chunks - 1)) return;
-    // stage 2 (last CTA of the tile): chunks summed in index order
+    if (s_ticket != last_ticket) return;
+    // stage 2 (last CTA of the tile): chunks (or group sums) added in index order
     __threadfence();
     {   // Small tiles (multi-lane layouts): all threads pull the tile's partials into the now idle stage buffers in
         // one round trip to L2, and the ordered sums read shared memory.  Same additions in the same order as the
         // direct path below, so the bits do not depend on which path runs.
         const int nvals = PT * 2 * NDET * a.n_chunks;
-        if (MULTI && nvals <= kStages * NP * kStageBins * 2) {
+        if (MULTI && a.n_groups == 1 && nvals <= kStages * NP * kStageBins * 2) {
             double *sh = reinterpret_cast<double *>(smem_raw);
             const double *src = a.partial + (tile * a.n_chunks * (int64_t)(2 * NDET)) * PT;
             for (int i = tid; i < nvals; i += kThreads) sh[i] = __ldcg(src + i);
@@ -814,30 +870,10 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             double sr[NDET], si[NDET];
 #pragma unroll
             for (int i = 0; i < NDET; ++i) { sr[i] = 0.0; si[i] = 0.0; }
-            const double *base = a.partial + (tile * a.n_chunks * (int64_t)(2 * NDET)) * PT + tid;
-            // loads of kFinishBatch chunks are issued together (the sum is latency-bound on L2 otherwise);
-            // the additions stay in chunk-index order, so the result does not depend on the batching.
-            constexpr int kFinishBatch = 8;
-            int c = 0;
-            for (; c + kFinishBatch <= a.n_chunks; c += kFinishBatch) {
-                double v[kFinishBatch][2 * NDET];
-#pragma unroll
-                for (int u = 0; u < kFinishBatch; ++u)
-#pragma unroll
-                    for (int q = 0; q < 2 * NDET; ++q)
-                        v[u][q] = __ldcg(base + ((int64_t)(c + u) * 2 * NDET + q) * PT);
-#pragma unroll
-                for (int u = 0; u < kFinishBatch; ++u)
-#pragma unroll
-                    for (int i = 0; i < NDET; ++i) { sr[i] += v[u][2 * i]; si[i] += v[u][2 * i + 1]; }
-            }
-            for (; c < a.n_chunks; ++c) {
-#pragma unroll
-                for (int i = 0; i < NDET; ++i) {
-                    sr[i] += __ldcg(base + ((int64_t)c * 2 * NDET + 2 * i) * PT);
-                    si[i] += __ldcg(base + ((int64_t)c * 2 * NDET + 2 * i + 1) * PT);
-                }
-            }
+            if (a.n_groups > 1)
+                ordered_sum(a.gpartial + (tile * a.n_groups * (int64_t)(2 * NDET)) * PT + tid, a.n_groups, sr, si);
+            else
+                ordered_sum(a.partial + (tile * a.n_chunks * (int64_t)(2 * NDET)) * PT + tid, a.n_chunks, sr, si);
             finish_proposal<NDET, ISCO>(a, bb, sr, si);
         }
     }
@@ -863,14 +899,15 @@ static cudaError_t launch_fused_t(const FusedArgs &a, int64_t blocks, cudaStream
 }
 
 cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, const double *rec,
-                         int64_t rec_stride, double *partial, unsigned int *tickets, double *lnl_out,
-                         double *parts_out, cudaStream_t s, int64_t *launches)
+                         int64_t rec_stride, double *partial, unsigned int *tickets, double *gpartial,
+                         unsigned int *gtickets, double *lnl_out, double *parts_out, cudaStream_t s, int64_t *launches)
 {
     FusedArgs a;
     a.planes = t.planes; a.rec = rec; a.n_pad = t.n_pad; a.n_bins = t.n_bins; a.n_prop = n_prop;
     a.rec_stride = rec_stride; a.n_chunks = plan.n_chunks; a.lpp = plan.lpp; a.f0 = t.f0; a.delta_f = t.delta_f;
     for (int i = 0; i < GW_MAX_DET; ++i) a.i7[i] = t.i7[i];
     a.partial = partial; a.tickets = tickets; a.lnl = lnl_out; a.parts = parts_out;
+    a.n_groups = plan.n_groups; a.gpartial = gpartial; a.gtickets = gtickets;
     const int64_t blocks = plan.n_tiles * plan.n_chunks;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     *launches += 1;
