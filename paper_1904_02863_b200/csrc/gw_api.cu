@@ -56,7 +56,7 @@ constexpr int64_t kMaxWaves = 8;
 #define GW_MULTI_PENALTY 1.35
 #endif
 constexpr double kMultiPenalty = GW_MULTI_PENALTY;     // the lanes-interleaved loop costs this much more per bin (measured, C2)
-constexpr double kFinishPerChunk = 0.25;   // last-CTA cross-chunk sum, in bin-sweep equivalents per chunk
+constexpr double kFinishPerChunk = 1.0;    // serial additions of the finish stage, in bin-sweep equivalents each (calibrated on C4 B = 256, 512)
 
 Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
 {
@@ -84,7 +84,9 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
             const double resident = (double)per_sm / (double)waves;           // average co-resident CTAs
             const double warps_per_sched = resident * (kThreads / 32) / 4.0;
             const double slowdown = warps_per_sched > kSatWarps ? warps_per_sched / kSatWarps : 1.0;
-            const double cost = (double)waves * per_thread * slowdown + kFinishPerChunk * (double)nc;
+            const double finish_len = nc >= kFinishTwoLevelFrom ? (double)(kFinishGroup + (nc + kFinishGroup - 1) / kFinishGroup)
+                                                                : (double)nc;   // serial additions of the finish
+            const double cost = (double)waves * per_thread * slowdown + kFinishPerChunk * finish_len;
             if (cost < best_cost) {
                 best_cost = cost;
                 best.lpp = lpp; best.props_per_cta = pt; best.n_chunks = (int)nc; best.n_tiles = tiles;
