@@ -157,6 +157,11 @@ int gw_ctx_info(const gw_ctx *ctx, int64_t *n_bins, int *n_det, double *delta_f,
 int gw_ctx_plan(const gw_ctx *ctx, int64_t n_prop, int *lanes_per_prop, int *props_per_cta,
                 int *n_chunks, int64_t *n_ctas);
 
+/* Testing / tuning aid: pin the launch shape gw_lnl_batch uses (lanes_per_prop in {1,2,4,8,16,32}, n_chunks >= 1
+ * frequency chunks per proposal tile); 0 leaves that choice to the planner.  A pinned shape whose partial sums do not
+ * fit the reserved workspace makes gw_lnl_batch return GW_ERR_INVALID_ARG.                              */
+int gw_ctx_force_plan(gw_ctx *ctx, int lanes_per_prop, int n_chunks);
+
 /* I7[n_det], the per-detector norm the precompute kernel produced (for tests of kernel K0).            */
 int gw_ctx_norms(const gw_ctx *ctx, double *i7_host);
 

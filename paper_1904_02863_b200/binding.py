@@ -24,7 +24,7 @@ GW_OK, GW_ERR_INVALID_ARG, GW_ERR_ALLOC, GW_ERR_CUDA, GW_ERR_ARCH = 0, -1, -2, -
 EXPORTS = (
     "gw_ctx_create", "gw_ctx_reserve", "gw_waveform_batch", "gw_lnl_batch", "gw_lnl_batch_host",
     "gw_waveform_batch_host", "gw_ctx_destroy", "gw_ctx_info", "gw_ctx_plan", "gw_ctx_norms",
-    "gw_ctx_launch_count", "gw_ctx_kernel_timing", "gw_ctx_last_kernel_ms", "gw_probe_fp64_fma_rate", "gw_strerror", "gw_last_cuda_error", "gw_abi_version",
+    "gw_ctx_launch_count", "gw_ctx_force_plan", "gw_ctx_kernel_timing", "gw_ctx_last_kernel_ms", "gw_probe_fp64_fma_rate", "gw_strerror", "gw_last_cuda_error", "gw_abi_version",
 )
 
 
@@ -78,6 +78,7 @@ def load_library():
     lib.gw_ctx_norms.argtypes = [vp, P(dbl)]
     lib.gw_ctx_launch_count.argtypes = [vp]
     lib.gw_ctx_launch_count.restype = i64
+    lib.gw_ctx_force_plan.argtypes = [vp, ci, ci]
     lib.gw_ctx_kernel_timing.argtypes = [vp, ci]
     lib.gw_ctx_last_kernel_ms.argtypes = [vp, P(dbl), P(dbl)]
     lib.gw_probe_fp64_fma_rate.argtypes = [ci, ci, P(dbl), P(dbl), vp]
@@ -210,6 +211,10 @@ class GwContext:
 
     def launch_count(self) -> int:
         return int(self._lib.gw_ctx_launch_count(self._h))
+
+    def force_plan(self, lanes_per_prop: int = 0, n_chunks: int = 0):
+        """Pin the launch shape of lnl_batch (0 = planner's choice); a testing / tuning aid."""
+        _check(self._lib.gw_ctx_force_plan(self._h, int(lanes_per_prop), int(n_chunks)), "gw_ctx_force_plan", self._h)
 
     def kernel_timing(self, enable: bool):
         _check(self._lib.gw_ctx_kernel_timing(self._h, int(bool(enable))), "gw_ctx_kernel_timing", self._h)

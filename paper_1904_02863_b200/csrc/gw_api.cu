@@ -22,6 +22,7 @@ struct gw_ctx {
     Workspace    w;
     int          last_cuda_error;
     int64_t      launches;
+    int          force_lpp, force_chunks;   // gw_ctx_force_plan (0 = planner's choice)
     int          timing;           // gw_ctx_kernel_timing: record events around K1 and the main kernel
     cudaEvent_t  ev[3];            // before K1, between K1 and main, after main
 };
@@ -67,6 +68,7 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
     Plan best = {1, kThreads, 1, (n_prop + kThreads - 1) / kThreads, 1};
     double best_cost = 1e300;
     for (int lpp = 1; lpp <= 32; lpp *= 2) {
+        if (ctx->force_lpp > 0 && lpp != ctx->force_lpp) continue;
         const int pt = kThreads / lpp;
         const int64_t tiles = (n_prop + pt - 1) / pt;
         int64_t max_chunks = M / ((int64_t)8 * lpp);          // at least 8 iterations per thread
@@ -74,7 +76,9 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
         if (max_chunks > by_waves) max_chunks = by_waves;
         if (max_chunks > kMaxChunks) max_chunks = kMaxChunks;
         if (max_chunks < 1) max_chunks = 1;
-        for (int64_t nc = 1; nc <= max_chunks; ++nc) {
+        int64_t nc_first = 1;
+        if (ctx->force_chunks > 0) { nc_first = max_chunks = (ctx->force_chunks < M ? ctx->force_chunks : M); }
+        for (int64_t nc = nc_first; nc <= max_chunks; ++nc) {
             const int64_t ctas = tiles * nc;
             const int64_t chunk = (M + nc - 1) / nc;
             const double per_thread = (double)((chunk + lpp - 1) / lpp) * (lpp > 1 ? kMultiPenalty : 1.0) + kProBins +
@@ -92,7 +96,7 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
                 best.lpp = lpp; best.props_per_cta = pt; best.n_chunks = (int)nc; best.n_tiles = tiles;
             }
         }
-        if (tiles >= slots) break;                            // enough proposals to fill the GPU: keep this lpp
+        if (tiles >= slots && ctx->force_lpp == 0) break;     // enough proposals to fill the GPU: keep this lpp
     }
     best.n_groups = best.n_chunks >= kFinishTwoLevelFrom ? (best.n_chunks + kFinishGroup - 1) / kFinishGroup : 1;
     return best;
@@ -359,6 +363,16 @@ int gw_ctx_plan(const gw_ctx *ctx, int64_t n_prop, int *lanes_per_prop, int *pro
     if (props_per_cta) *props_per_cta = p.props_per_cta;
     if (n_chunks) *n_chunks = p.n_chunks;
     if (n_ctas) *n_ctas = p.n_tiles * p.n_chunks;
+    return GW_OK;
+}
+
+int gw_ctx_force_plan(gw_ctx *ctx, int lanes_per_prop, int n_chunks)
+{
+    if (!ctx || n_chunks < 0) return GW_ERR_INVALID_ARG;
+    if (lanes_per_prop != 0 && (lanes_per_prop < 1 || lanes_per_prop > 32 || (lanes_per_prop & (lanes_per_prop - 1)) != 0))
+        return GW_ERR_INVALID_ARG;
+    ctx->force_lpp = lanes_per_prop;
+    ctx->force_chunks = n_chunks;
     return GW_OK;
 }
 

@@ -78,15 +78,27 @@ def test_lnl_all_lane_layouts(oracle, torch_cuda, batch):
     assert plan["lanes_per_prop"] * plan["props_per_cta"] == 256
 
 
-def test_lane_layouts_cover_all_widths(oracle, torch_cuda):
-    """The planner reaches every lane width 1..32 somewhere in the sweep used above (so the test above covers them)."""
-    cfg = inputs.CONFIGS["C1"].reduced(f_max=301.25, batch=600)
+@pytest.mark.parametrize("lpp", [1, 2, 4, 8, 16, 32])
+@pytest.mark.parametrize("n_chunks", [1, 3, 40])
+def test_every_lane_width_and_chunking_forced(oracle, torch_cuda, lpp, n_chunks):
+    """gw_ctx_force_plan pins the launch shape, so every lanes-per-proposal layout is exercised with one chunk (direct
+    finish), a few chunks (single-level finish) and 40 chunks (two-level finish), whatever the planner would choose."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=301.25, batch=100)        # 1126 bins
     f, S, dets, d, th = make_problem(oracle, cfg)
-    seen = set()
-    with make_ctx(cfg, f, d, S, dets, max_batch=70000) as ctx:
-        for b in [1, 2, 3, 7, 8, 9, 16, 31, 33, 64, 100, 255, 257, 600, 4096, 70000]:
-            seen.add(ctx.plan(b)["lanes_per_prop"])
-    assert 1 in seen and 32 in seen and len(seen) >= 3, seen
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        ctx.force_plan(lpp, n_chunks)
+        plan = ctx.plan(100)
+        assert plan["lanes_per_prop"] == lpp and plan["n_chunks"] == n_chunks
+        lnl, parts = ctx.lnl_batch(_dev(torch, th), want_parts=True)
+        again = ctx.lnl_batch(_dev(torch, th))
+        torch.cuda.synchronize()
+        assert torch.equal(lnl, again)
+        lnl, parts = lnl.cpu().numpy(), parts.cpu().numpy()
+        ctx.force_plan(0, 0)
+        assert ctx.plan(100)["lanes_per_prop"] * ctx.plan(100)["props_per_cta"] == 256
+    lnl_ref, parts_ref, _ = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th, cfg.spin_order)
+    assert_lnl_close(lnl, parts, lnl_ref, parts_ref)
 
 
 @pytest.mark.parametrize("n_det", [1, 2, 4])
