@@ -50,7 +50,8 @@ bool is_device_ptr(const void *p)
 // about kSatWarps warps per scheduler.  The plan is a pure function of (n_prop, M, n_det, device), which is
 // what makes the summation order reproducible.
 constexpr double kProBins  = 14.0;
-constexpr double kSatWarps = 3.0;
+constexpr double kSatWarps = 2.0;     // one 8-warp CTA per SM (2 warps per scheduler) already reaches the fp64 pipe's rate (measured)
+constexpr double kCoResidentGain = 0.985;
 constexpr int    kMaxChunks = 4096;
 constexpr int64_t kMaxWaves = 8;
 #ifndef GW_MULTI_PENALTY
@@ -87,7 +88,8 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
             const int64_t waves = (per_sm + slots_per_sm - 1) / slots_per_sm;
             const double resident = (double)per_sm / (double)waves;           // average co-resident CTAs
             const double warps_per_sched = resident * (kThreads / 32) / 4.0;
-            const double slowdown = warps_per_sched > kSatWarps ? warps_per_sched / kSatWarps : 1.0;
+            double slowdown = warps_per_sched > kSatWarps ? warps_per_sched / kSatWarps : 1.0;
+            if (resident >= 2.0) slowdown *= kCoResidentGain;  // a second CTA hides the first one's stage boundaries
             const double finish_len = nc >= kFinishTwoLevelFrom ? (double)(kFinishGroup + (nc + kFinishGroup - 1) / kFinishGroup)
                                                                 : (double)nc;   // serial additions of the finish
             const double cost = (double)waves * per_thread * slowdown + kFinishPerChunk * finish_len;
