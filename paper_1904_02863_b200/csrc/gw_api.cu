@@ -50,14 +50,22 @@ bool is_device_ptr(const void *p)
 // about kSatWarps warps per scheduler.  The plan is a pure function of (n_prop, M, n_det, device), which is
 // what makes the summation order reproducible.
 constexpr double kProBins  = 14.0;
-constexpr double kSatWarps = 2.0;     // one 8-warp CTA per SM (2 warps per scheduler) already reaches the fp64 pipe's rate (measured)
+#ifndef GW_SAT_WARPS
+#define GW_SAT_WARPS 2.0
+#endif
+#ifndef GW_EXCLUSIVE_PLANS
+#define GW_EXCLUSIVE_PLANS 1
+#endif
+constexpr double kSatWarps = GW_SAT_WARPS;   // one 8-warp CTA per SM nearly saturates the fp64 pipe (brute-force sweep)
 constexpr double kCoResidentGain = 0.985;
+constexpr double kCoResidentGainMulti = 0.90;   // the lanes-interleaved loop (shuffles, short chunks) gains more from a second CTA (C0)
 constexpr int    kMaxChunks = 4096;
 constexpr int64_t kMaxWaves = 8;
 #ifndef GW_MULTI_PENALTY
 #define GW_MULTI_PENALTY 1.35
 #endif
 constexpr double kMultiPenalty = GW_MULTI_PENALTY;     // the lanes-interleaved loop costs this much more per bin (measured, C2)
+constexpr double kTwoLevelHop = 16.0;      // the second fence + ticket round of the two-level finish (~2 us; C4 B = 1, 16)
 constexpr double kFinishPerChunk = 1.0;    // serial additions of the finish stage, in bin-sweep equivalents each (calibrated on C4 B = 256, 512)
 
 Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
@@ -66,7 +74,7 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
     const int slots_per_sm = ctx->ctas_per_sm > 0 ? ctx->ctas_per_sm : 1;
     const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 148;
     const int64_t slots = (int64_t)n_sm * slots_per_sm;
-    Plan best = {1, kThreads, 1, (n_prop + kThreads - 1) / kThreads, 1};
+    Plan best = {1, kThreads, 1, (n_prop + kThreads - 1) / kThreads, 1, 0};
     double best_cost = 1e300;
     for (int lpp = 1; lpp <= 32; lpp *= 2) {
         if (ctx->force_lpp > 0 && lpp != ctx->force_lpp) continue;
@@ -82,20 +90,24 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
         for (int64_t nc = nc_first; nc <= max_chunks; ++nc) {
             const int64_t ctas = tiles * nc;
             const int64_t chunk = (M + nc - 1) / nc;
-            const double per_thread = (double)((chunk + lpp - 1) / lpp) * (lpp > 1 ? kMultiPenalty : 1.0) + kProBins +
-                                      (lpp > 1 ? 2.0 : 0.0);
+            const double sweep = (double)((chunk + lpp - 1) / lpp) * (lpp > 1 ? kMultiPenalty : 1.0);
+            const double pro = kProBins + (lpp > 1 ? 2.0 : 0.0);
             const int64_t per_sm = (ctas + n_sm - 1) / n_sm;                  // CTAs an SM must run
             const int64_t waves = (per_sm + slots_per_sm - 1) / slots_per_sm;
             const double resident = (double)per_sm / (double)waves;           // average co-resident CTAs
             const double warps_per_sched = resident * (kThreads / 32) / 4.0;
             double slowdown = warps_per_sched > kSatWarps ? warps_per_sched / kSatWarps : 1.0;
-            if (resident >= 2.0) slowdown *= kCoResidentGain;  // a second CTA hides the first one's stage boundaries
-            const double finish_len = nc >= kFinishTwoLevelFrom ? (double)(kFinishGroup + (nc + kFinishGroup - 1) / kFinishGroup)
+            if (resident >= 2.0) slowdown *= (lpp > 1 ? kCoResidentGainMulti : kCoResidentGain);  // a second CTA hides the first one's stage boundaries
+            const double finish_len = nc >= kFinishTwoLevelFrom ? kTwoLevelHop + (double)(kFinishGroup + (nc + kFinishGroup - 1) / kFinishGroup)
                                                                 : (double)nc;   // serial additions of the finish
-            const double cost = (double)waves * per_thread * slowdown + kFinishPerChunk * finish_len;
+            // lanes-interleaved CTAs have short sweeps and a latency-bound prologue that a co-resident CTA covers
+            const double per_cta = lpp > 1 ? sweep * slowdown + pro : (sweep + pro) * slowdown;
+            const double cost = (double)waves * per_cta + kFinishPerChunk * finish_len;
             if (cost < best_cost) {
                 best_cost = cost;
                 best.lpp = lpp; best.props_per_cta = pt; best.n_chunks = (int)nc; best.n_tiles = tiles;
+                // a grid that fits one CTA per SM is launched so that no SM takes two (launch_fused)
+                best.exclusive = (GW_EXCLUSIVE_PLANS && ctas <= n_sm) ? 1 : 0;
             }
         }
         if (tiles >= slots && ctx->force_lpp == 0) break;     // enough proposals to fill the GPU: keep this lpp

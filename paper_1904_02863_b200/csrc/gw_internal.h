@@ -36,6 +36,7 @@ constexpr int kBasis      = 8;     // per-bin phase basis values (4 planes of 2)
 constexpr int kBasisPlanes = 5;    // (x^-5,x^-3) (x^-2,x^-1) (ln f,x) (x ln f,x^2) (f,f^-7/6)
 constexpr int kFinishGroup = 16;   // chunks per group of the two-level finish
 constexpr int kFinishTwoLevelFrom = 33;  // n_chunks from which the finish is two-level
+constexpr int kExclusiveSmemBytes = 120 * 1024;   // > half of an SM's 228 KB: at most one such CTA per SM
 constexpr int kRecFixed   = 10;    // record fields before the per-detector block
 constexpr int kRecPerDet  = 5;     // tau, Cre, Cim, rot_re, rot_im
 // record fields: 0..8 phase coefficients, then kRecPerDet per detector, then f_ISCO and the index of the last
@@ -72,6 +73,7 @@ struct Plan {
     int     n_chunks;     // frequency chunks per proposal tile
     int64_t n_tiles;      // ceil(n_prop / props_per_cta)
     int     n_groups;     // 1, or ceil(n_chunks / kFinishGroup) when the finish is two-level
+    int     exclusive;    // 1: the grid has at most one CTA per SM and is launched so that no SM takes two
 };
 
 struct Workspace {

@@ -885,12 +885,21 @@ size_t fused_smem_bytes(int n_det)
     return (size_t)kStages * (kBasisPlanes + n_det) * kStageBins * sizeof(double2) + kStages * sizeof(uint64_t);
 }
 
+// A grid of at most one CTA per SM must not land two CTAs on one SM while another kernel (the setup kernel under
+// programmatic dependent launch, or the previous call's tail) still holds some SMs: the doubled-up SMs would take
+// twice as long.  Asking for more than half of an SM's shared memory makes the placement one per SM.
+size_t fused_smem_bytes_exclusive(int n_det)
+{
+    const size_t need = fused_smem_bytes(n_det), half = (size_t)kExclusiveSmemBytes;
+    return need > half ? need : half;
+}
+
 template <int NDET, bool MULTI, bool ISCO>
-static cudaError_t launch_fused_t(const FusedArgs &a, int64_t blocks, cudaStream_t s)
+static cudaError_t launch_fused_t(const FusedArgs &a, int64_t blocks, bool exclusive, cudaStream_t s)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)blocks); cfg.blockDim = dim3(kThreads);
-    cfg.dynamicSmemBytes = fused_smem_bytes(NDET); cfg.stream = s;
+    cfg.dynamicSmemBytes = exclusive ? fused_smem_bytes_exclusive(NDET) : fused_smem_bytes(NDET); cfg.stream = s;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
@@ -913,12 +922,13 @@ cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, cons
     *launches += 1;
     a.i7cum = t.i7cum; a.phase_marginal = t.phase_marginal;
     const int variant = (plan.lpp > 1 ? 1 : 0) + (t.isco_cut ? 2 : 0);
+    const bool ex = plan.exclusive != 0;
 #define GW_DISPATCH(N)                                                                      \
     switch (variant) {                                                                      \
-    case 0: return launch_fused_t<N, false, false>(a, blocks, s);                           \
-    case 1: return launch_fused_t<N, true, false>(a, blocks, s);                            \
-    case 2: return launch_fused_t<N, false, true>(a, blocks, s);                            \
-    default: return launch_fused_t<N, true, true>(a, blocks, s);                            \
+    case 0: return launch_fused_t<N, false, false>(a, blocks, ex, s);                           \
+    case 1: return launch_fused_t<N, true, false>(a, blocks, ex, s) ;                            \
+    case 2: return launch_fused_t<N, false, true>(a, blocks, ex, s) ;                            \
+    default: return launch_fused_t<N, true, true>(a, blocks, ex, s);                            \
     }
     switch (t.n_det) {
     case 1: GW_DISPATCH(1)
@@ -935,7 +945,7 @@ static int g_ctas_per_sm[GW_MAX_DET + 1] = {0, 0, 0, 0, 0};
 template <int NDET>
 static cudaError_t configure_one()
 {
-    const int smem = (int)fused_smem_bytes(NDET);
+    const int smem = (int)fused_smem_bytes_exclusive(NDET);
     cudaError_t e;
     e = cudaFuncSetAttribute(fused_kernel<NDET, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
@@ -946,7 +956,7 @@ static cudaError_t configure_one()
     e = cudaFuncSetAttribute(fused_kernel<NDET, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     int n = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fused_kernel<NDET, false, false>, kThreads, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fused_kernel<NDET, false, false>, kThreads, fused_smem_bytes(NDET));
     if (e != cudaSuccess) return e;
     g_ctas_per_sm[NDET] = n > 0 ? n : 1;
     return cudaSuccess;
