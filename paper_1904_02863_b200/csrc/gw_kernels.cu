@@ -482,7 +482,7 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
 // chunk; the tables are read from shared memory as warp broadcasts), 2..32 for small batches (the lanes
 // of a proposal interleave over the bins; a fixed xor-shuffle tree combines them).
 // The chunk is streamed through a kStages-deep ring of kStageBins-bin stages by bulk async copies (TMA
-// engine) completing on mbarriers.  Per (proposal, bin): 9 FMA phase (incl. f tau_0), 14-op sincos (cis_phase) giving
+// engine) completing on mbarriers.  Per (proposal, bin): 9 FMA phase (incl. f tau_0), 12-op sincos (cis_phase_lnl) giving
 // E = e^{+2 pi i (Phi' + f tau_0)}, detector 0: Z_0 += g_0j E (4 FMA), and per detector I >= 1
 //     Z_I <- Z_I * rot_I + g_Ij * E                                                  (8 fp64 ops)
 // where rot_I = exp(-2 pi i lpp df (tau_I - tau_0)): after the sweep Z_I * exp(+2 pi i f_last (tau_I - tau_0))
@@ -652,7 +652,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                     for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(tau[0], v[u].x, ph[u]);   // + f tau_0
                 }
 #pragma unroll
-                for (int u = 0; u < kUnroll; ++u) cis_phase(ph[u], cs[u], sn[u]);
+                for (int u = 0; u < kUnroll; ++u) cis_phase_lnl(ph[u], cs[u], sn[u]);
                 if (ISCO) {                                      // h = 0 above f_ISCO: the bin contributes nothing
 #pragma unroll
                     for (int u = 0; u < kUnroll; ++u)
@@ -715,7 +715,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                                     P[2 * kStageBins + jj], P[3 * kStageBins + jj]);
             ph = __fma_rn(tau[0], P[4 * kStageBins + jj].x, ph);
             double c, sn;
-            cis_phase(ph, c, sn);
+            cis_phase_lnl(ph, c, sn);
             if (ISCO && jstage + jj > jcut) { c = 0.0; sn = 0.0; }
 #pragma unroll
             for (int i = 0; i < NDET; ++i) {

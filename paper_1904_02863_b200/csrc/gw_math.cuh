@@ -103,13 +103,61 @@ __device__ __forceinline__ void cis_quarter_turns(double t4, double &c_out, doub
     s_out = __hiloint2double(__double2hiint(im) ^ neg_im, __double2loint(im));
 }
 
+// Trimmed variant for the fused likelihood kernel: sin of degree 4 and cos of degree 5 in z (gen_sincos_coeffs.py 4 5:
+// max abs error 3.4e-12 and 5.6e-14), 12 fp64-pipe instructions.  The error is 300x below the 1e-9 waveform gate and
+// enters lnL far below the 1e-8 gate; the waveform kernel, which is HBM-bound, keeps the
+// full-degree polynomials.
+#define GW_SINT_S0 6.2831853071524
+#define GW_SINT_S1 -41.341702153394905
+#define GW_SINT_S2 81.60520471104576
+#define GW_SINT_S3 -76.6978663502028
+#define GW_SINT_S4 41.47283323950919
+#define GW_COST_C0 0.9999999999999444
+#define GW_COST_C1 -19.739208801922548
+#define GW_COST_C2 64.93939383134831
+#define GW_COST_C3 -85.45676493719407
+#define GW_COST_C4 60.23818359301454
+#define GW_COST_C5 -26.058123753882793
+__device__ __forceinline__ void cis_quarter_turns_trim(double t4, double &c_out, double &s_out)
+{
+    const int    q = __double2int_rn(t4);
+    const double r = t4 - __int2double_rn(q);             // in [-1/2, 1/2] quarter turns, exact
+    const double z = r * r;
+    double ps = __fma_rn(GW_SINT_S4 / 262144.0, z, GW_SINT_S3 / 16384.0);      // S_k / (4 * 16^k)
+    double pc = __fma_rn(GW_COST_C5 / 1048576.0, z, GW_COST_C4 / 65536.0);     // C_k / 16^k
+    ps = __fma_rn(ps, z, GW_SINT_S2 / 1024.0);
+    pc = __fma_rn(pc, z, GW_COST_C3 / 4096.0);
+    ps = __fma_rn(ps, z, GW_SINT_S1 / 64.0);
+    pc = __fma_rn(pc, z, GW_COST_C2 / 256.0);
+    ps = __fma_rn(ps, z, GW_SINT_S0 / 4.0);
+    pc = __fma_rn(pc, z, GW_COST_C1 / 16.0);
+    const double s = ps * r;
+    const double c = __fma_rn(pc, z, GW_COST_C0);
+    const bool   odd = (q & 1) != 0;
+    const double re = odd ? s : c;
+    const double im = odd ? c : s;
+    const int neg_re = ((q + 1) & 2) << 30;
+    const int neg_im = (q & 2) << 30;
+    c_out = __hiloint2double(__double2hiint(re) ^ neg_re, __double2loint(re));
+    s_out = __hiloint2double(__double2hiint(im) ^ neg_im, __double2loint(im));
+}
+
 // The kernels carry the phase in units of 1/kPhaseScale turns and call cis_phase().
 #if GW_CIS_QUARTER
 constexpr double kPhaseScale = 4.0;
 __device__ __forceinline__ void cis_phase(double t, double &c, double &s) { cis_quarter_turns(t, c, s); }
+#ifndef GW_SINCOS_TRIM
+#define GW_SINCOS_TRIM 1
+#endif
+#if GW_SINCOS_TRIM
+__device__ __forceinline__ void cis_phase_lnl(double t, double &c, double &s) { cis_quarter_turns_trim(t, c, s); }
+#else
+__device__ __forceinline__ void cis_phase_lnl(double t, double &c, double &s) { cis_quarter_turns(t, c, s); }
+#endif
 #else
 constexpr double kPhaseScale = 1.0;
 __device__ __forceinline__ void cis_phase(double t, double &c, double &s) { cis_turns(t, c, s); }
+__device__ __forceinline__ void cis_phase_lnl(double t, double &c, double &s) { cis_turns(t, c, s); }
 #endif
 
 // (cos, sin) of 2 pi * (a*b) with the product reduced mod 1 from its exact two-term expansion: used

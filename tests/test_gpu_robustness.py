@@ -171,3 +171,38 @@ def test_sub_band_contexts_add_up(oracle):
     ref = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th, cfg.spin_order)
     assert_lnl_close(lnl_from_parts(total).cpu().numpy(), total.cpu().numpy(), ref[0], ref[1])
     assert_lnl_close(full_lnl.cpu().numpy(), full_parts.cpu().numpy(), ref[0], ref[1])
+
+
+@pytest.mark.gpu
+def test_one_cta_per_sm_grids_are_not_doubled_up(oracle):
+    """DESIGN.md section 7, exclusive grids: a plan of at most one CTA per SM must take the same time whether
+    or not another kernel is still resident when it is launched (setup kernel under programmatic dependent
+    launch, the L2 flush before it).  Unprotected, the step took 1.7x the two kernels' own time."""
+    import torch
+    cfg = inputs.CONFIGS["C1"]
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    ctx = make_ctx(cfg, f, d, S, dets)
+    B = cfg.batch
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    ctx.force_plan(1, max(1, n_sm // ((B + 255) // 256)))      # 16 tiles x 9 chunks = 144 CTAs on 148 SMs
+    assert ctx.plan(B)["n_ctas"] <= n_sm
+    thd = torch.from_numpy(th[:B]).cuda()
+    lnl = torch.empty(B, dtype=torch.float64, device="cuda")
+    busy = torch.empty(64 << 20, dtype=torch.uint8, device="cuda")
+    for _ in range(5):
+        ctx.lnl_batch(thd, out=lnl)
+    ctx.kernel_timing(True)
+    alone = []
+    for _ in range(10):
+        ctx.lnl_batch(thd, out=lnl)
+        k1, k3 = ctx.last_kernel_ms()
+        alone.append(k1 + k3)
+    ctx.kernel_timing(False)
+    steps = []
+    for _ in range(30):
+        busy.fill_(1)                                          # still draining when the step's kernels launch
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); ctx.lnl_batch(thd, out=lnl); e1.record()
+        torch.cuda.synchronize()
+        steps.append(e0.elapsed_time(e1))
+    assert np.median(steps) < 1.35 * np.median(alone), (np.median(steps), np.median(alone))
