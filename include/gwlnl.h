@@ -179,7 +179,8 @@ int gw_ctx_last_kernel_ms(gw_ctx *ctx, double *setup_ms, double *main_ms);
  * per SM): enqueues `n_iter` rounds of 64 instructions per thread and reports achieved fp64 FMA/s -- the measured
  * roofline denominator (MEASURED_PEAKS.json has no fp64 entry).  `mode` selects the operand pattern:
  * 0 = fma(v, imm, imm) (pipe peak); 1 = fma(a, b, v) with three distinct register operands; 2 = three register
- * operands of which one is shared by consecutive instructions; 3 = mma.sync m8n8k4 f64.  Synchronises.
+ * operands of which one is shared by consecutive instructions; 3 = mma.sync m8n8k4 f64; 4, 5 = mode 0 with 8 or 16
+ * independent integer instructions beside every 8 DFMA (does the fp64 rate drop?).  Synchronises.
  * Errors: GW_ERR_INVALID_ARG, GW_ERR_CUDA, GW_ERR_ARCH.                                                 */
 int gw_probe_fp64_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, void *cuda_stream);
 

@@ -525,7 +525,7 @@ int gw_waveform_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host
 
 int gw_probe_fp64_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, void *cuda_stream)
 {
-    if (n_iter < 1 || mode < 0 || mode > 3) return GW_ERR_INVALID_ARG;
+    if (n_iter < 1 || mode < 0 || mode > 5) return GW_ERR_INVALID_ARG;
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return GW_ERR_CUDA;

@@ -993,12 +993,21 @@ __global__ void __launch_bounds__(256) fma_probe_kernel(int n_iter, const double
         v[i] = in[threadIdx.x + i]; a[i] = in[64 + threadIdx.x + 3 * i]; b[i] = in[128 + threadIdx.x + 5 * i];
     }
     const double m = in[7];
+    unsigned int x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = threadIdx.x * 2654435761u + i;
     for (int it = 0; it < n_iter; ++it) {
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
+            // modes 4, 5: independent integer instructions (one IMAD + one LOP3 per element) beside the 8 DFMA:
+            // are their issue slots free?
+            if (MODE == 4 || MODE == 5) {
+#pragma unroll
+                for (int i = 0; i < (MODE == 4 ? 4 : 8); ++i) x[i] = (x[i] ^ (unsigned)it) * 3u + 0x9e3779b9u;
+            }
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                if (MODE == 0) v[i] = __fma_rn(v[i], 0.999999, 1e-9);
+                if (MODE == 0 || MODE == 4 || MODE == 5) v[i] = __fma_rn(v[i], 0.999999, 1e-9);
                 if (MODE == 1) v[i] = __fma_rn(a[i], b[i], v[i]);
                 if (MODE == 2) v[i] = __fma_rn(a[i], m, v[i]);
                 if (MODE == 3)
@@ -1010,6 +1019,12 @@ __global__ void __launch_bounds__(256) fma_probe_kernel(int n_iter, const double
     double r = 0.0;
 #pragma unroll
     for (int i = 0; i < 8; ++i) r += v[i] + b[i];
+    if (MODE == 4 || MODE == 5) {
+        unsigned int y = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) y ^= x[i];
+        if (y == 0x12345u) r = 123.456;
+    }
     if (r == 123.456) sink[0] = r;                           // never true; keeps the chains alive
 }
 
@@ -1030,6 +1045,8 @@ cudaError_t probe_fma_rate(int n_iter, int mode, double *fma_per_s, double *elap
         case 1:  fma_probe_kernel<1><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
         case 2:  fma_probe_kernel<2><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
         case 3:  fma_probe_kernel<3><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        case 4:  fma_probe_kernel<4><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        case 5:  fma_probe_kernel<5><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
         default: fma_probe_kernel<0><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
         }
     };

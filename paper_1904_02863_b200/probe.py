@@ -7,7 +7,9 @@ from .binding import probe_fp64_fma_rate
 
 MODES = {0: "fma(v, imm, imm): one register operand", 1: "fma(a, b, v): three distinct register operands",
          2: "fma(a, m, v): three register operands, one shared by consecutive instructions",
-         3: "mma.sync m8n8k4 f64 (DMMA)"}
+         3: "mma.sync m8n8k4 f64 (DMMA)",
+         4: "mode 0 plus 8 independent integer instructions per 8 DFMA (do other pipes issue for free?)",
+         5: "mode 0 plus 16 independent integer instructions per 8 DFMA"}
 
 
 def main():
