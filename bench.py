@@ -264,7 +264,13 @@ def run_ours(args):
     ctx.kernel_timing(False)
     fused_ms = float(np.mean(k_ms))
     walg = walg_per_bin(n_det)
-    flops_per_launch = 2.0 * walg * B * M
+    pairs = float(B) * M                                   # (proposal, bin) pairs with algorithmic work
+    if args.isco_cut:                                      # only bins up to each proposal's f_ISCO carry work
+        from paper_1904_02863_b200.inputs import P_MC, P_Q
+        m_tot = th[:, P_MC] * (1.0 + th[:, P_Q]) ** 1.2 / th[:, P_Q] ** 0.6
+        f_isco = 1.0 / (6.0 ** 1.5 * np.pi * m_tot * 4.925490947641267e-06)
+        pairs = float(np.searchsorted(f, f_isco, side="right").sum())
+    flops_per_launch = 2.0 * walg * pairs
     achieved = flops_per_launch / (fused_ms * 1e-3) / 1e12
     peaks = {}
     try:
@@ -280,7 +286,7 @@ def run_ours(args):
                                % (n_sm, FP64_LANES_PER_SM, sm_max,
                                   "MEASURED_PEAKS.json sm_max_mhz" if "sm_max_mhz" in peaks else "fallback clock, B200_PROFILING.md"),
                 "peak_measured_fma_probe": 2 * fma_rate / 1e12, "frac_of_measured": achieved / (2 * fma_rate / 1e12),
-                "flop_per_launch": flops_per_launch, "walg_fma_per_prop_bin": walg,
+                "flop_per_launch": flops_per_launch, "walg_fma_per_prop_bin": walg, "proposal_bin_pairs": pairs,
                 "kernel_ms": fused_ms, "setup_kernel_ms": float(np.mean(s_ms))}
 
     # ---- end to end: host buffers through gw_lnl_batch_host (H2D + kernels + D2H + sync inside the call) ----

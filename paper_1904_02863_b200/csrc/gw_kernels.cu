@@ -581,9 +581,11 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             bulk_g2s(sm + (size_t)(buf * NP + p) * kStageBins, src + (int64_t)p * a.n_pad, bytes, &bars[buf]);
     };
 
+    __shared__ int s_relmax;
     if (tid == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&bars[s], 1);
         mbar_fence_init();
+        s_relmax = -1;
     }
     __syncthreads();
     if (tid == 0)
@@ -602,15 +604,33 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
     }
 
     int64_t jcut = 0;
-    if (ISCO) jcut = (int64_t)a.rec[(int64_t)rec_field_jcut(NDET) * a.rec_stride + b];
+    int n_run = n_stage;                                     // stages this CTA sweeps
+    if (ISCO) {
+        // Stages wholly above the cut-off of every proposal of the CTA contribute nothing: they are neither loaded
+        // (beyond the prefetched ones) nor swept.  The rotation recurrence stops with the last swept bin, which is
+        // the f_last of the seed below.
+        jcut = (int64_t)a.rec[(int64_t)rec_field_jcut(NDET) * a.rec_stride + b];
+        int rel = (int)max((int64_t)-1, min(jcut - j0, (int64_t)n - 1));
+        rel = __reduce_max_sync(0xffffffffu, rel);
+        if (lane == 0) atomicMax(&s_relmax, rel);
+        __syncthreads();
+        n_run = s_relmax < 0 ? 0 : s_relmax / kStageBins + 1;
+    }
     int iters_total = 0;
     for (int s = 0; s < n_stage; ++s) {
         const int buf = s % kStages;
         const int cnt = min(kStageBins, n - s * kStageBins);
+        if (ISCO && s >= n_run) {                            // drain the prefetched stages, then stop
+            if (s >= kStages) break;
+            mbar_wait(&bars[buf], 0u);
+            continue;
+        }
         mbar_wait(&bars[buf], (uint32_t)((s / kStages) & 1));
         const double2 *P = sm + (size_t)buf * NP * kStageBins;
         const int iters = MULTI ? (cnt + lpp - 1) / lpp : cnt;
         const int64_t jstage = j0 + (int64_t)s * kStageBins;  // global index of the stage's first bin
+        // last kept bin of this proposal relative to the stage (isco_cut), in [-1, kStageBins]
+        const int cut_local = ISCO ? (int)max((int64_t)-1, min(jcut - jstage, (int64_t)kStageBins)) : 0;
         int it = 0;
         if (!MULTI) {
             // kUnroll bins per trip, written plane by plane ("k-major"): consecutive fp64 instructions then
@@ -656,7 +676,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                 if (ISCO) {                                      // h = 0 above f_ISCO: the bin contributes nothing
 #pragma unroll
                     for (int u = 0; u < kUnroll; ++u)
-                        if (jstage + it + u > jcut) { cs[u] = 0.0; sn[u] = 0.0; }
+                        if (it + u > cut_local) { cs[u] = 0.0; sn[u] = 0.0; }
                 }
             };
             auto update_z = [&](int it, const double (&cs)[kUnroll], const double (&sn)[kUnroll]) {
@@ -716,7 +736,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             ph = __fma_rn(tau[0], P[4 * kStageBins + jj].x, ph);
             double c, sn;
             cis_phase_lnl(ph, c, sn);
-            if (ISCO && jstage + jj > jcut) { c = 0.0; sn = 0.0; }
+            if (ISCO && jj > cut_local) { c = 0.0; sn = 0.0; }
 #pragma unroll
             for (int i = 0; i < NDET; ++i) {
                 double2 g = P[(kBasisPlanes + i) * kStageBins + jj];
@@ -735,7 +755,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
         }
         iters_total += iters;
         __syncthreads();                                     // every warp is done with this buffer
-        if (tid == 0 && s + kStages < n_stage) issue_stage(s + kStages);
+        if (tid == 0 && s + kStages < n_run) issue_stage(s + kStages);
     }
 
     // seed (detectors >= 1): multiply by exp(+2 pi i f_last (tau_I - tau_0)), f_last = frequency of this

@@ -52,6 +52,30 @@ def test_isco_cut_all_lane_layouts(oracle, batch):
     assert_lnl_close(lnl.cpu().numpy(), parts.cpu().numpy(), ref[0], ref[1])
 
 
+@pytest.mark.parametrize("lpp,n_chunks", [(1, 1), (1, 7), (1, 40), (4, 3), (8, 40), (32, 11)])
+def test_isco_cut_skipped_stages_in_forced_plans(oracle, lpp, n_chunks):
+    """Stages (and whole CTAs) above every proposal's cut-off are not swept (fused_kernel, ISCO): BBH proposals cut at
+    45-110 Hz in a band up to 1024 Hz, so with 7 or 40 chunks most CTAs sweep nothing and the CTA holding the cut
+    sweeps part of its stages; one light proposal (cut above the band) per tile keeps every stage of that tile alive
+    in the second half of the batch."""
+    import torch
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=1024.0, batch=520)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    th = th.copy()
+    th[300:, inputs.P_MC] = np.where(np.arange(300, 520) % 64 == 0, 1.2, th[300:, inputs.P_MC])   # f_ISCO > 1024 Hz
+    with _ctx(cfg, f, d, S, dets, isco_cut=1) as ctx:
+        ctx.force_plan(lpp, n_chunks)
+        plan = ctx.plan(len(th))
+        assert plan["lanes_per_prop"] == lpp and plan["n_chunks"] == n_chunks
+        thd = torch.from_numpy(th).cuda()
+        lnl, parts = ctx.lnl_batch(thd, want_parts=True)
+        again, _ = ctx.lnl_batch(thd, want_parts=True)
+        torch.cuda.synchronize()
+    ref = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th, cfg.spin_order, isco_cut=1)
+    assert_lnl_close(lnl.cpu().numpy(), parts.cpu().numpy(), ref[0], ref[1])
+    assert torch.equal(lnl, again)
+
+
 @pytest.mark.parametrize("isco", [0, 1])
 def test_phase_marginal(oracle, isco):
     import torch
