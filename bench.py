@@ -37,7 +37,7 @@ FP64_LANES_PER_SM = 64          # B200 fp64 FMA lanes per S
 L2_FLUSH_BYTES = 256 << 20
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/*_fused_ncu_summary.md); None where no capture exists for the workload.
-NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 1.82e6, "C2": 33.46e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 1.82e6, "C2": 33.47e6}
 
 
 def parse_workload(spec):
