@@ -44,12 +44,23 @@ bool is_device_ptr(const void *p)
     return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
 }
 
+// device alias of pinned (mapped) host memory, or nullptr for pageable host memory
+double *mapped_alias(const void *host_ptr)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, host_ptr) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return at.type == cudaMemoryTypeHost ? static_cast<double *>(at.devicePointer) : nullptr;
+}
+
 // ---- launch planning -----------------------------------------------------------------------------------
 // Cost model: a CTA sweeps ceil(chunk/lpp) bins per thread plus a fixed prologue /
 // epilogue worth ~kProBins bins; an SM runs its resident CTAs concurrently and the fp64 pipe saturates at
 // about kSatWarps warps per scheduler.  The plan is a pure function of (n_prop, M, n_det, device), which is
 // what makes the summation order reproducible.
 constexpr double kProBins  = 14.0;
+#ifndef GW_ZERO_COPY_LNL
+#define GW_ZERO_COPY_LNL 1
+#endif
 #ifndef GW_SAT_WARPS
 #define GW_SAT_WARPS 2.0
 #endif
@@ -478,9 +489,17 @@ int gw_lnl_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, dou
     cudaError_t e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * GW_NPARAM,
                                     cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
-    rc = gw_lnl_batch(ctx, n_prop, w.theta_stage, w.lnl_stage, parts_out_host ? w.parts_stage : nullptr, cuda_stream);
+    // lnL goes straight to a pinned output buffer (coalesced 8-byte stores of the finish stage over the host link):
+    // one copy-engine round trip less per call; pageable buffers and `parts` take the staged copy
+#if GW_ZERO_COPY_LNL
+    double *direct = mapped_alias(lnl_out_host);
+#else
+    double *direct = nullptr;
+#endif
+    rc = gw_lnl_batch(ctx, n_prop, w.theta_stage, direct ? direct : w.lnl_stage, parts_out_host ? w.parts_stage : nullptr,
+                      cuda_stream);
     if (rc != GW_OK) return rc;
-    e = cudaMemcpyAsync(lnl_out_host, w.lnl_stage, sizeof(double) * n_prop, cudaMemcpyDeviceToHost, s);
+    if (!direct) e = cudaMemcpyAsync(lnl_out_host, w.lnl_stage, sizeof(double) * n_prop, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess && parts_out_host)
         e = cudaMemcpyAsync(parts_out_host, w.parts_stage, sizeof(double) * n_prop * ctx->t.n_det * 3,
                             cudaMemcpyDeviceToHost, s);

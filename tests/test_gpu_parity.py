@@ -193,6 +193,26 @@ def test_host_variants_match_device_variants(oracle, torch_cuda):
     assert np.array_equal(h_h, h_d.cpu().numpy()) and np.array_equal(lnl_only, lnl_h)
 
 
+@pytest.mark.parametrize("batch", [1, 130, 1500])
+def test_host_variant_with_pinned_output(oracle, torch_cuda, batch):
+    """A pinned lnL buffer is written by the kernel itself (include/gwlnl.h, host variants): same bits as the staged
+    copy into a pageable buffer, nothing outside the n_prop entries is touched, and a sub-array offset works."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=200.0, batch=1500)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    th = th[:batch]
+    with make_ctx(cfg, f, d, S, dets) as ctx:
+        staged = ctx.lnl_batch_host(th)                                   # pageable numpy output
+        pinned = torch.full((batch + 16,), -7.0, dtype=torch.float64).pin_memory()
+        view = pinned.numpy()[8:8 + batch]
+        th_pin = torch.from_numpy(th.copy()).pin_memory()
+        got, parts = ctx.lnl_batch_host(th_pin.numpy(), out=view, want_parts=True)
+        again = ctx.lnl_batch_host(th_pin.numpy(), out=view)
+    assert np.array_equal(view, staged) and np.array_equal(again, staged)
+    assert np.all(pinned.numpy()[:8] == -7.0) and np.all(pinned.numpy()[8 + batch:] == -7.0)
+    assert np.isfinite(parts).all()
+
+
 def test_device_resident_context_inputs(oracle, torch_cuda):
     """gw_ctx_create accepts device pointers for freqs / data / psd."""
     torch = torch_cuda
