@@ -1,5 +1,7 @@
 """`-m gpu`: the CUDA path (through the C-ABI of include/gwlnl.h) against the CPU oracle, element by element,
 on the same seeded inputs (SURVEY.md section 9 gates 2-4; tolerances from BASELINE.json north_star)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -326,7 +328,7 @@ def test_time_shift_interchange(oracle, torch_cuda):
     np.testing.assert_allclose(np.abs(ha), np.abs(hb), rtol=1e-12)
 
 
-@pytest.mark.parametrize("seed", range(24))
+@pytest.mark.parametrize("seed", range(int(os.environ.get("GW_RANDOM_SHAPES", "24"))))   # soak: GW_RANDOM_SHAPES=500
 def test_random_shapes(oracle, torch_cuda, seed):
     """Seeded random shapes: bins 2..2500, proposals 1..700, 1..4 detectors (geometric and fixed mixed), random band,
     resolution, mass range and options -- ragged tails everywhere the launch planner can put one."""
@@ -378,8 +380,13 @@ def test_random_shapes(oracle, torch_cuda, seed):
     keep = hh > 0                                     # isco_cut below the band: h = 0, lnL = 0 exactly
     assert np.all(lnl[~keep] == 0) and np.all(parts[~keep] == 0)
     if keep.any():
+        # Gate A16 plus the conditioning term of DESIGN.md section 8: the fp64 phase of either side is defined to
+        # ~1e-11 rad (a few ulp of its largest term), and a phase offset dphi moves Re<d|h> by |<d|h>| dphi, which
+        # the A16 scale does not cover when the signal is buried (<h|h> << |Im<d|h>|; soak seed 444: 3 bins,
+        # <h|h> = 4e-7, |<d|h>| = 6e-4).  dphi = 1e-10 rad.
         scale = np.abs(parts_ref[keep][..., 0].sum(axis=1)) + hh[keep]
-        assert (np.abs(lnl[keep] - lnl_ref[keep]) / scale).max() <= 1e-8
+        modulus = np.hypot(parts_ref[keep][..., 0].sum(axis=1), parts_ref[keep][..., 1].sum(axis=1))
+        assert np.all(np.abs(lnl[keep] - lnl_ref[keep]) <= 1e-8 * scale + 1e-10 * modulus)
         pscale = (np.hypot(parts_ref[keep][..., 0], parts_ref[keep][..., 1]) + parts_ref[keep][..., 2])[..., None]
         ok = pscale[..., 0] > 0
         assert (np.abs(parts[keep] - parts_ref[keep])[ok] / pscale[ok]).max() <= 1e-8
