@@ -333,7 +333,7 @@ def test_random_shapes(oracle, torch_cuda, seed):
     """Seeded random shapes: bins 2..2500, proposals 1..700, 1..4 detectors (geometric and fixed mixed), random band,
     resolution, mass range and options -- ragged tails everywhere the launch planner can put one."""
     torch = torch_cuda
-    from paper_1904_02863_b200 import GwContext
+    from paper_1904_02863_b200 import GwContext, GwError
     rng = np.random.Generator(np.random.PCG64(4242 + seed))
     n_det = int(rng.integers(1, 5))
     M = int(rng.choice([2, 3, 5, 31, 33, 127, 129, 257, 640, 1000, 2500]))
@@ -367,9 +367,19 @@ def test_random_shapes(oracle, torch_cuda, seed):
     gmst = float(rng.uniform(0, 2 * np.pi))
     z = rng.standard_normal((n_det, M, 2))
     d = oracle.waveform(f, dets, gmst, th[:1], spin)[0] + (z[..., 0] + 1j * z[..., 1]) * np.sqrt(S / (4 * df))
+    rng2 = np.random.Generator(np.random.PCG64(777 + seed))          # every other case: a pinned launch shape
     with GwContext(f, d, S, dets, gmst, spin_order=spin, max_batch=B, isco_cut=isco, phase_marginal=marg) as ctx:
         thd = _dev(torch, th)
-        lnl, parts = ctx.lnl_batch(thd, want_parts=True)
+        if rng2.random() < 0.5:
+            lpp = int(rng2.choice([1, 2, 4, 8, 16, 32]))
+            ctx.force_plan(lpp, int(rng2.integers(1, max(2, min(80, M // lpp + 1)))))
+            try:
+                lnl, parts = ctx.lnl_batch(thd, want_parts=True)
+            except GwError:                                          # shape does not fit the reserved workspace
+                ctx.force_plan(0, 0)
+                lnl, parts = ctx.lnl_batch(thd, want_parts=True)
+        else:
+            lnl, parts = ctx.lnl_batch(thd, want_parts=True)
         h = ctx.waveform_batch(thd[: min(B, 16)].contiguous())
         torch.cuda.synchronize()
         lnl, parts, h = lnl.cpu().numpy(), parts.cpu().numpy(), h.cpu().numpy()
