@@ -206,3 +206,43 @@ def test_one_cta_per_sm_grids_are_not_doubled_up(oracle):
         torch.cuda.synchronize()
         steps.append(e0.elapsed_time(e1))
     assert np.median(steps) < 1.35 * np.median(alone), (np.median(steps), np.median(alone))
+
+
+@pytest.mark.parametrize("seed", range(3))
+def test_call_sequences_leave_no_state_behind(oracle, seed):
+    """Tickets, group tickets and partial sums are reused from call to call (self-resetting counters): a random
+    sequence of batch sizes and pinned launch shapes on ONE context must give, call by call, the bits a fresh
+    context gives for the same call."""
+    import torch
+    from paper_1904_02863_b200 import GwError
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=332.5, batch=700)        # 1251 bins
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    rng = np.random.Generator(np.random.PCG64(9000 + seed))
+    calls = []
+    for _ in range(40):
+        B = int(rng.choice([1, 3, 8, 31, 64, 200, 256, 257, 512, 700]))
+        lpp = int(rng.choice([0, 1, 2, 4, 8, 16, 32]))
+        nc = 0 if lpp == 0 else int(rng.choice([1, 2, 5, 16, 33, 40, 70]))
+        calls.append((B, lpp, nc))
+    thd = torch.from_numpy(th).cuda()
+
+    def run(ctx, B, lpp, nc):
+        ctx.force_plan(lpp, nc)
+        try:
+            out, parts = ctx.lnl_batch(thd[:B].contiguous(), want_parts=True)
+        except GwError:
+            return None
+        torch.cuda.synchronize()
+        return out.cpu().numpy(), parts.cpu().numpy()
+
+    with make_ctx(cfg, f, d, S, dets, max_batch=700) as shared:
+        got = [run(shared, *c) for c in calls]
+    n_checked = 0
+    for c, g in zip(calls, got):
+        with make_ctx(cfg, f, d, S, dets, max_batch=700) as fresh:
+            want = run(fresh, *c)
+        assert (g is None) == (want is None), c
+        if g is not None:
+            assert np.array_equal(g[0], want[0]) and np.array_equal(g[1], want[1]), c
+            n_checked += 1
+    assert n_checked >= 20
