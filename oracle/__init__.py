@@ -57,6 +57,12 @@ def _load():
     lib.gwo_waveform_opt.argtypes = [i64, dp, cint, dp, dbl, i64, dp, cint, cint, dp]
     lib.gwo_lnl_opt.argtypes = [i64, dp, dbl, cint, dp, dp, dp, dbl, i64, dp, cint, cint, cint, dp, dp]
     lib.gwo_lnl_opt.restype = cint
+    lib.gwo_tidal_coefficients.argtypes = [dbl, dbl, dbl, cint, dp, dp]
+    lib.gwo_phase_tidal.argtypes = [dbl, dp, cint, dp, cint]
+    lib.gwo_phase_tidal.restype = dbl
+    lib.gwo_waveform_tidal.argtypes = [i64, dp, cint, dp, dbl, i64, dp, cint, cint, dp, cint, dp]
+    lib.gwo_lnl_tidal.argtypes = [i64, dp, dbl, cint, dp, dp, dp, dbl, i64, dp, cint, cint, dp, cint, cint, dp, dp]
+    lib.gwo_lnl_tidal.restype = cint
     lib.gwo_f_isco.argtypes = [dbl, dbl]
     lib.gwo_f_isco.restype = dbl
     lib.gwo_log_bessel_i0.argtypes = [dbl]
@@ -108,11 +114,22 @@ def phase_coefficients(eta, mu1, mu2, chi1=0.0, chi2=0.0, spin_order=1):
     return phi, phil
 
 
-def phase(freqs, theta, spin_order=1) -> np.ndarray:
-    """O3: Psi(f) for one theta[11] at each frequency."""
+def phase(freqs, theta, spin_order=1, lambdas=None, tidal_order=0) -> np.ndarray:
+    """O3: Psi(f) for one theta[11] at each frequency (tidal option: lambdas = (Lambda_1, Lambda_2))."""
     lib = _load()
     th = _f64(theta, (NPARAM,))
-    return np.array([lib.gwo_phase(float(f), _p(th), spin_order) for f in np.atleast_1d(freqs)])
+    if lambdas is None or tidal_order == 0:
+        return np.array([lib.gwo_phase(float(f), _p(th), spin_order) for f in np.atleast_1d(freqs)])
+    lam = _f64(lambdas, (2,))
+    return np.array([lib.gwo_phase_tidal(float(f), _p(th), spin_order, _p(lam), int(tidal_order))
+                     for f in np.atleast_1d(freqs)])
+
+
+def tidal_coefficients(eta, lambda1, lambda2, tidal_order=2):
+    """NEXT-1 option -> (phi_10, phi_12) in units of 3/(128 eta) v^(k-5)."""
+    a, b = ctypes.c_double(), ctypes.c_double()
+    _load().gwo_tidal_coefficients(eta, lambda1, lambda2, int(tidal_order), ctypes.byref(a), ctypes.byref(b))
+    return a.value, b.value
 
 
 def amplitude(mc: float, dl: float) -> float:
@@ -135,18 +152,28 @@ def sky_frame(ra, dec, psi, gmst):
     return X, Y, n
 
 
-def waveform(freqs, dets, gmst, theta, spin_order=1, isco_cut=0) -> np.ndarray:
-    """O4..O6: h[n_prop][n_det][n_bins] complex128 (isco_cut=1: zero above f_ISCO, NEXT-1 option)."""
+def _lambdas(lambdas, n_prop, tidal_order):
+    if lambdas is None or tidal_order == 0:
+        return None, None, 0
+    lam = _f64(lambdas).reshape(n_prop, 2)
+    return lam, _p(lam), int(tidal_order)
+
+
+def waveform(freqs, dets, gmst, theta, spin_order=1, isco_cut=0, lambdas=None, tidal_order=0) -> np.ndarray:
+    """O4..O6: h[n_prop][n_det][n_bins] complex128 (isco_cut=1: zero above f_ISCO; lambdas[n_prop][2] with
+    tidal_order 1 | 2: 5PN | 5PN + 6PN tidal phase terms -- NEXT-1 options)."""
     f = _f64(freqs)
     d = _f64(dets).reshape(-1, DET_ROW)
     th = _f64(theta).reshape(-1, NPARAM)
     out = np.empty((th.shape[0], d.shape[0], f.shape[0], 2))
-    _load().gwo_waveform_opt(f.shape[0], _p(f), d.shape[0], _p(d), gmst, th.shape[0], _p(th),
-                             spin_order, int(isco_cut), _p(out))
+    lam, lam_p, order = _lambdas(lambdas, th.shape[0], tidal_order)
+    _load().gwo_waveform_tidal(f.shape[0], _p(f), d.shape[0], _p(d), gmst, th.shape[0], _p(th),
+                               spin_order, int(isco_cut), lam_p, order, _p(out))
     return out.view(np.complex128)[..., 0]
 
 
-def lnl(freqs, delta_f, data, psd, dets, gmst, theta, spin_order=1, n_threads=0, isco_cut=0):
+def lnl(freqs, delta_f, data, psd, dets, gmst, theta, spin_order=1, n_threads=0, isco_cut=0,
+        lambdas=None, tidal_order=0):
     """O7 -> (lnL[n_prop], parts[n_prop][n_det][3], threads_used)."""
     f = _f64(freqs)
     d = _f64(dets).reshape(-1, DET_ROW)
@@ -156,8 +183,10 @@ def lnl(freqs, delta_f, data, psd, dets, gmst, theta, spin_order=1, n_threads=0,
     th = _f64(theta).reshape(-1, NPARAM)
     out = np.empty(th.shape[0])
     parts = np.empty((th.shape[0], n_det, 3))
-    used = _load().gwo_lnl_opt(n_bins, _p(f), float(delta_f), n_det, _p(dat), _p(S), _p(d), gmst,
-                               th.shape[0], _p(th), spin_order, int(isco_cut), int(n_threads), _p(out), _p(parts))
+    lam, lam_p, order = _lambdas(lambdas, th.shape[0], tidal_order)
+    used = _load().gwo_lnl_tidal(n_bins, _p(f), float(delta_f), n_det, _p(dat), _p(S), _p(d), gmst,
+                                 th.shape[0], _p(th), spin_order, int(isco_cut), lam_p, order, int(n_threads),
+                                 _p(out), _p(parts))
     return out, parts, used
 
 

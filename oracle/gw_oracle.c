@@ -36,7 +36,9 @@
  * Cauchy-Schwarz (P3), shift identities (P4), antenna-pattern invariants and a
  * closed-form special case (P5), light-travel-time bounds (P6), 40-digit
  * mpmath spot values (P7), a hand-expanded tiny case (P8), bin independence
- * (P9).  The digits of the H1/L1/V1 geometry are input data, not oracle
+ * (P9); the tidal option (NEXT-1): Lambda~ form against the per-body form, re-derivation from the tidal
+ * energy and flux, equal-mass special case, 40-digit spot values (P10, tests/test_oracle_tidal.py).
+ * The digits of the H1/L1/V1 geometry are input data, not oracle
  * arithmetic; they are pinned by invariants only.
  */
 #include <complex.h>
@@ -113,6 +115,35 @@ void gwo_phase_coefficients(double eta, double mu1, double mu2, double chi1, dou
     phi[7] = pi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * eta * eta);
 }
 
+/* ---- NEXT-1 option: tidal phase terms ------------------------ */
+/* Point-mass TaylorF2 plus the adiabatic quadrupolar tidal terms, for the neutron-star workloads C2/C3
+ * (the paper's motivation includes the neutron-star equation of state; the formula is not in
+ * PAPER.md -- literature closed form, reading A21).  With Lambda_A = (2/3) k2_A (R_A/m_A)^5 the dimensionless
+ * tidal deformability of body A (body 1 is the heavier one, q = m2/m1 <= 1),
+ *   Lambda~  = (8/13) [ (1 + 7 eta - 31 eta^2)(L1 + L2) + sqrt(1-4 eta)(1 + 9 eta - 11 eta^2)(L1 - L2) ]
+ *   dLambda~ = (1/2) [ sqrt(1-4 eta)(1 - 13272/1319 eta + 8944/1319 eta^2)(L1 + L2)
+ *                     + (1 - 15910/1319 eta + 32850/1319 eta^2 + 3380/1319 eta^3)(L1 - L2) ]
+ *   phi_10 = -(39/2) Lambda~                                            (5PN, tidal_order >= 1)
+ *   phi_12 = -(3115/64) Lambda~ + (6595/364) sqrt(1-4 eta) dLambda~     (6PN, tidal_order >= 2)
+ * in the same units as phi_0..phi_7: Psi += 3/(128 eta) v^-5 (phi_10 v^10 + phi_12 v^12).
+ * tidal_order 0: both are zero.                                                                     */
+void gwo_tidal_coefficients(double eta, double lambda1, double lambda2, int tidal_order,
+                            double *phi10, double *phi12)
+{
+    *phi10 = 0.0;
+    *phi12 = 0.0;
+    if (tidal_order <= 0) return;
+    const double root = sqrt(fmax(0.0, 1.0 - 4.0 * eta));
+    const double ls = lambda1 + lambda2, la = lambda1 - lambda2;
+    const double lam_t = 8.0 / 13.0 * ((1.0 + 7.0 * eta - 31.0 * eta * eta) * ls
+                                       + root * (1.0 + 9.0 * eta - 11.0 * eta * eta) * la);
+    const double dlam_t = 0.5 * (root * (1.0 - 13272.0 / 1319.0 * eta + 8944.0 / 1319.0 * eta * eta) * ls
+                                 + (1.0 - 15910.0 / 1319.0 * eta + 32850.0 / 1319.0 * eta * eta
+                                    + 3380.0 / 1319.0 * eta * eta * eta) * la);
+    *phi10 = -39.0 / 2.0 * lam_t;
+    if (tidal_order >= 2) *phi12 = -3115.0 / 64.0 * lam_t + 6595.0 / 364.0 * root * dlam_t;
+}
+
 /* ---- O3: phase at one frequency ------------------------------------------------------- */
 /* Psi(f) = 2 pi f t_c - phi_c - pi/4 + 3/(128 eta) v^-5 sum_k (phi_k + phil_k ln v) v^k,
  * v = (pi M_s f)^(1/3).  No cut-off at f_ISCO (reading A6).
@@ -120,6 +151,7 @@ void gwo_phase_coefficients(double eta, double mu1, double mu2, double chi1, dou
  * over bins compute them once per proposal and pass them in.                                 */
 typedef struct {
     double eta, mtot_s, phi[8], phil[8], tc, phic;
+    double phi10, phi12;          /* tidal option; zero otherwise */
 } gwo_source;
 
 static gwo_source source_of(const double *theta, int spin_order)
@@ -130,6 +162,17 @@ static gwo_source source_of(const double *theta, int spin_order)
     gwo_phase_coefficients(s.eta, mu1, mu2, theta[T_CHI1], theta[T_CHI2], spin_order, s.phi, s.phil);
     s.tc = theta[T_TC];
     s.phic = theta[T_PHIC];
+    s.phi10 = 0.0;
+    s.phi12 = 0.0;
+    return s;
+}
+
+/* the same with the tidal option: lambdas = (Lambda_1, Lambda_2) of this proposal, or NULL */
+static gwo_source source_of_tidal(const double *theta, int spin_order, const double *lambdas, int tidal_order)
+{
+    gwo_source s = source_of(theta, spin_order);
+    if (lambdas && tidal_order > 0)
+        gwo_tidal_coefficients(s.eta, lambdas[0], lambdas[1], tidal_order, &s.phi10, &s.phi12);
     return s;
 }
 
@@ -142,6 +185,8 @@ static double phase_of(const gwo_source *s, double f)
         series += (s->phi[k] + s->phil[k] * lnv) * vk;
         vk *= v;
     }
+    if (s->phi10 != 0.0 || s->phi12 != 0.0)        /* tidal option: v^10 and v^12 terms */
+        series += s->phi10 * pow(v, 10.0) + s->phi12 * pow(v, 12.0);
     return 2.0 * GWO_PI * f * s->tc - s->phic - GWO_PI / 4.0
          + 3.0 / (128.0 * s->eta) * pow(v, -5.0) * series;
 }
@@ -149,6 +194,12 @@ static double phase_of(const gwo_source *s, double f)
 double gwo_phase(double f, const double *theta, int spin_order)
 {
     gwo_source s = source_of(theta, spin_order);
+    return phase_of(&s, f);
+}
+
+double gwo_phase_tidal(double f, const double *theta, int spin_order, const double *lambdas, int tidal_order)
+{
+    gwo_source s = source_of_tidal(theta, spin_order, lambdas, tidal_order);
     return phase_of(&s, f);
 }
 
@@ -230,14 +281,16 @@ static double complex h_det_at(double f, const gwo_source *src, double cosi,
 }
 
 /* h_out[n_prop][n_det][n_bins][2] (re, im) */
-void gwo_waveform_opt(int64_t n_bins, const double *freqs, int n_det, const double *dets, double gmst,
-                      int64_t n_prop, const double *theta, int spin_order, int isco_cut, double *h_out)
+/* lambdas: NULL, or [n_prop][2] = (Lambda_1, Lambda_2) per proposal, used when tidal_order > 0 */
+void gwo_waveform_tidal(int64_t n_bins, const double *freqs, int n_det, const double *dets, double gmst,
+                        int64_t n_prop, const double *theta, int spin_order, int isco_cut,
+                        const double *lambdas, int tidal_order, double *h_out)
 {
 #pragma omp parallel for schedule(dynamic, 1)
     for (int64_t b = 0; b < n_prop; ++b) {
         const double *th = theta + b * T_N;
         const double a0 = gwo_amplitude(th[T_MC], th[T_DL]);
-        const gwo_source src = source_of(th, spin_order);
+        const gwo_source src = source_of_tidal(th, spin_order, lambdas ? lambdas + 2 * b : NULL, tidal_order);
         const double f_cut = isco_cut ? gwo_f_isco(th[T_MC], th[T_Q]) : 0.0;
         for (int i = 0; i < n_det; ++i) {
             double fp, fc, dt;
@@ -265,10 +318,10 @@ static void neumaier_add(double *sum, double *comp, double x)
 /* data_ri[n_det][n_bins][2], psd[n_det][n_bins]; lnl[n_prop]; parts[n_prop][n_det][3] =
  * (Re<d|h>, Im<d|h>, <h|h>) (parts may be NULL).  n_threads <= 0: OpenMP default.
  * Returns the number of threads the proposal loop used.                                        */
-int gwo_lnl_opt(int64_t n_bins, const double *freqs, double delta_f, int n_det,
-                const double *data_ri, const double *psd, const double *dets, double gmst,
-                int64_t n_prop, const double *theta, int spin_order, int isco_cut, int n_threads,
-                double *lnl, double *parts)
+int gwo_lnl_tidal(int64_t n_bins, const double *freqs, double delta_f, int n_det,
+                  const double *data_ri, const double *psd, const double *dets, double gmst,
+                  int64_t n_prop, const double *theta, int spin_order, int isco_cut,
+                  const double *lambdas, int tidal_order, int n_threads, double *lnl, double *parts)
 {
     int used = 1;
 #ifdef _OPENMP
@@ -280,7 +333,7 @@ int gwo_lnl_opt(int64_t n_bins, const double *freqs, double delta_f, int n_det,
     for (int64_t b = 0; b < n_prop; ++b) {
         const double *th = theta + b * T_N;
         const double a0 = gwo_amplitude(th[T_MC], th[T_DL]);
-        const gwo_source src = source_of(th, spin_order);
+        const gwo_source src = source_of_tidal(th, spin_order, lambdas ? lambdas + 2 * b : NULL, tidal_order);
         const double f_cut = isco_cut ? gwo_f_isco(th[T_MC], th[T_Q]) : 0.0;
         double total = 0.0;
         for (int i = 0; i < n_det; ++i) {
@@ -309,6 +362,21 @@ int gwo_lnl_opt(int64_t n_bins, const double *freqs, double delta_f, int n_det,
         lnl[b] = total;
     }
     return used;
+}
+
+/* the point-mass entry points (no tidal terms) */
+void gwo_waveform_opt(int64_t n_bins, const double *freqs, int n_det, const double *dets, double gmst,
+                      int64_t n_prop, const double *theta, int spin_order, int isco_cut, double *h_out)
+{
+    gwo_waveform_tidal(n_bins, freqs, n_det, dets, gmst, n_prop, theta, spin_order, isco_cut, NULL, 0, h_out);
+}
+int gwo_lnl_opt(int64_t n_bins, const double *freqs, double delta_f, int n_det,
+                const double *data_ri, const double *psd, const double *dets, double gmst,
+                int64_t n_prop, const double *theta, int spin_order, int isco_cut, int n_threads,
+                double *lnl, double *parts)
+{
+    return gwo_lnl_tidal(n_bins, freqs, delta_f, n_det, data_ri, psd, dets, gmst, n_prop, theta, spin_order,
+                         isco_cut, NULL, 0, n_threads, lnl, parts);
 }
 
 /* the default (no cut-off) entry points, as pinned by tests/test_oracle_*.py */

@@ -179,6 +179,16 @@ def proposals(cfg: Config, batch: Optional[int] = None) -> np.ndarray:
     return np.ascontiguousarray(th)
 
 
+def tidal_lambdas(cfg: Config, batch: Optional[int] = None, lam_max: float = 5000.0) -> np.ndarray:
+    """lambdas[B][2]: dimensionless tidal deformabilities (Lambda_1, Lambda_2) ~ U[0, lam_max] for the tidal option
+    (NEXT-1; the usual prior range of neutron-star analyses), drawn from a stream of their own so that the
+    11-column proposals above are unchanged.  Row 0 (the injection's slot) is (400, 600)."""
+    rng = np.random.Generator(np.random.PCG64(cfg.seed_prop + 5))
+    lam = lam_max * rng.random((cfg.batch, 2))
+    lam[0, :] = (400.0, 600.0)
+    return np.ascontiguousarray(lam if batch is None else lam[:batch])
+
+
 def noise(cfg: Config) -> np.ndarray:
     """n[n_det][M] complex: Re and Im each N(0, S/(4 delta_f)), independent per detector and bin."""
     rng = np.random.Generator(np.random.PCG64(cfg.seed_noise))
