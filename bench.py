@@ -48,9 +48,10 @@ def parse_workload(spec):
     return name, cfg, batch
 
 
-def walg_per_bin(n_det):
-    """Algorithmic fp64 FMA-equivalents per (proposal, bin): SURVEY.md 8(d) W_alg = 31 + 8 N_det."""
-    return 31 + 8 * n_det
+def walg_per_bin(n_det, tidal_order=0):
+    """Algorithmic fp64 FMA-equivalents per (proposal, bin): SURVEY.md 8(d) W_alg = 31 + 8 N_det; the tidal
+    option adds x^5 (t10 + t12 x^2) from the tabulated x, x^2: 4 more."""
+    return 31 + 8 * n_det + (4 if tidal_order else 0)
 
 
 class ClockSampler:
@@ -104,8 +105,9 @@ class ClockSampler:
         return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def build_problem(cfg, batch_total):
-    """freqs, data, psd, det rows, theta[batch_total] -- the injection comes from the library's own waveform."""
+def build_problem(cfg, batch_total, tidal_order=0):
+    """freqs, data, psd, det rows, theta[batch_total] -- the injection comes from the library's own waveform.
+    With the tidal option theta has 13 columns (seeded Lambda_1, Lambda_2 appended; the injection stays point-mass)."""
     from dataclasses import replace
     from paper_1904_02863_b200 import binding, inputs
     f = inputs.frequency_grid(cfg)
@@ -114,24 +116,31 @@ def build_problem(cfg, batch_total):
     d = inputs.make_data(cfg, binding.waveform_for_inputs)
     draw = max(cfg.batch, batch_total)
     th = inputs.proposals(replace(cfg, batch=draw))[:batch_total]
+    if tidal_order:
+        th = np.ascontiguousarray(np.hstack([th, inputs.tidal_lambdas(replace(cfg, batch=draw))[:batch_total]]))
     return f, S, dets, d, th
 
 
-def oracle_rate(cfg, f, S, dets, d, th, target_s, n_threads=0):
+def oracle_rate(cfg, f, S, dets, d, th, target_s, n_threads=0, tidal_order=0):
     """Time the oracle, as it stands, for about target_s seconds of wall time on a bounded sample of the
     workload: a prefix of the proposals, passed over repeatedly if the whole batch is quicker than target_s."""
     import oracle
     oracle.build()
+
+    def run(rows):
+        kw = dict(lambdas=rows[:, 11:13], tidal_order=tidal_order) if tidal_order else {}
+        return oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, rows[:, :11], cfg.spin_order, n_threads, **kw)
+
     pilot = th[: min(len(th), max(2, 2 * (os.cpu_count() or 1)))]
-    oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, pilot, cfg.spin_order, n_threads)      # thread start-up
+    run(pilot)                                                                              # thread start-up
     t0 = time.perf_counter()
-    oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, pilot, cfg.spin_order, n_threads)
+    run(pilot)
     dt = max(time.perf_counter() - t0, 1e-6)
     n = int(min(len(th), max(len(pilot), len(pilot) * target_s / dt)))
     passes = max(1, int(round(target_s / max(dt * n / len(pilot), 1e-6))))
     t0 = time.perf_counter()
     for _ in range(passes):
-        _, _, used = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:n], cfg.spin_order, n_threads)
+        _, _, used = run(th[:n])
     dt = time.perf_counter() - t0
     return n * passes / dt, used, n, dt, passes
 
@@ -194,7 +203,7 @@ def run_ours(args):
     n_gpus = world
 
     name, cfg, batch = parse_workload(args.workload)
-    f, S, dets, d, th_all = build_problem(cfg, batch * world)
+    f, S, dets, d, th_all = build_problem(cfg, batch * world, args.tidal_order)
     from paper_1904_02863_b200.sharding import shard_range
     lo, hi = shard_range(batch * world, rank, world)
     th = np.ascontiguousarray(th_all[lo:hi])
@@ -202,7 +211,8 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
 
     ctx = GwContext(f, d, S, dets, cfg.gmst, spin_order=cfg.spin_order, max_batch=B,
-                    isco_cut=int(args.isco_cut), phase_marginal=int(args.phase_marginal))
+                    isco_cut=int(args.isco_cut), phase_marginal=int(args.phase_marginal),
+                    tidal_order=int(args.tidal_order))
     thd = torch.from_numpy(th).cuda()
     lnl = torch.empty(B, dtype=torch.float64, device="cuda")
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
@@ -263,7 +273,7 @@ def run_ours(args):
         k_ms.append(b)
     ctx.kernel_timing(False)
     fused_ms = float(np.mean(k_ms))
-    walg = walg_per_bin(n_det)
+    walg = walg_per_bin(n_det, args.tidal_order)
     pairs = float(B) * M                                   # (proposal, bin) pairs with algorithmic work
     if args.isco_cut:                                      # only bins up to each proposal's f_ISCO carry work
         from paper_1904_02863_b200.inputs import P_MC, P_Q
@@ -358,10 +368,12 @@ def run_ours(args):
     # ---- CPU baseline: the oracle as it stands on this box's host cores (rank 0, N = 1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        rate, used, n, dt, passes = oracle_rate(cfg, f, S, dets, d, th, args.cpu_seconds, n_threads=os.cpu_count() or 1)
+        rate, used, n, dt, passes = oracle_rate(cfg, f, S, dets, d, th, args.cpu_seconds, n_threads=os.cpu_count() or 1,
+                                                    tidal_order=args.tidal_order)
         cpu = {"value": rate, "unit": UNIT, "cores": used, "kind": "oracle",
                "sample": f"first {n} of {B} proposals x {passes} passes, all {M} bins x {n_det} detectors, {dt:.1f} s wall"}
-        r1, u1, n1, dt1, p1 = oracle_rate(cfg, f, S, dets, d, th, min(3.0, args.cpu_seconds), n_threads=1)
+        r1, u1, n1, dt1, p1 = oracle_rate(cfg, f, S, dets, d, th, min(3.0, args.cpu_seconds), n_threads=1,
+                                              tidal_order=args.tidal_order)
         cpu["single_thread"] = {"value": r1, "cores": u1, "sample": f"first {n1} proposals x {p1} passes, {dt1:.1f} s wall"}
 
     clocks = clk.summary()
@@ -373,7 +385,8 @@ def run_ours(args):
                 "config": {"workload": f"{name}: {n_det} det x {M} bins x {B} proposals per GPU",
                            "global_batch": B * world, "bins": M, "detectors": n_det, "parallelism": f"proposals sharded x{world}",
                            "l2": "flushed before every timed step: 256 MiB write, then a 256 MiB read of a second buffer (no dirty lines left)", "plan": plan,
-                           "options": {"isco_cut": int(args.isco_cut), "phase_marginal": int(args.phase_marginal)}},
+                           "options": {"isco_cut": int(args.isco_cut), "phase_marginal": int(args.phase_marginal),
+                                       "tidal_order": int(args.tidal_order)}},
                 "bin_det_proposals_per_s": value * M * n_det,
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
                 "roofline": roofline, "cpu_baseline": cpu}
@@ -395,6 +408,8 @@ def main():
     ap.add_argument("--no-waveform", action="store_true")
     ap.add_argument("--isco-cut", action="store_true", help="NEXT-1 option: h = 0 above f_ISCO (not the headline config)")
     ap.add_argument("--phase-marginal", action="store_true", help="NEXT-1 option: lnL marginalised over phi_c")
+    ap.add_argument("--tidal-order", type=int, default=0, choices=[0, 1, 2],
+                    help="NEXT-1 option: 5PN (1) or 5PN + 6PN (2) tidal phase terms; theta rows of 13 columns")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -49,7 +49,7 @@
 extern "C" {
 #endif
 
-#define GW_ABI_VERSION 2
+#define GW_ABI_VERSION 3
 
 enum {
     GW_OK              =  0,
@@ -74,7 +74,7 @@ typedef struct gw_detector {
     double fplus, fcross, dt_s;  /* FIXED: response and time delay (seconds)                              */
 } gw_detector;
 
-typedef struct gw_options {      /* NULL => { spin_order 1, isco_cut 0, max_batch 4096, phase_marginal 0 } */
+typedef struct gw_options {      /* NULL => { spin_order 1, isco_cut 0, max_batch 4096, phase_marginal 0, tidal_order 0 } */
     int     spin_order;          /* 0: no spin terms; 1: 1.5PN spin-orbit + 2PN spin-spin (A7)  */
     int     isco_cut;            /* 0 (default, A6): every bin of the band is evaluated;
                                     1 (NEXT-1 option): h = 0 for f > f_ISCO =
@@ -83,7 +83,8 @@ typedef struct gw_options {      /* NULL => { spin_order 1, isco_cut 0, max_batc
     int     phase_marginal;      /* 0: lnL at the proposal's phi_c; 1 (NEXT-1 option): lnl_out holds the
                                     likelihood marginalised over phi_c with a uniform prior,
                                     ln I0(|sum_I <d|h>_I|) - 1/2 sum_I <h|h>_I; parts are unchanged        */
-    int     reserved;            /* must be 0                                                              */
+    int     tidal_order;         /* 0: point masses; 1 | 2 (NEXT-1 option): 5PN | 5PN + 6PN
+                                    adiabatic tidal phase terms; theta rows then have GW_NPARAM_TIDAL columns  */
 } gw_options;
 
 /* Column order of one proposal theta[GW_NPARAM] (units: Msun, -, -, -, Mpc, s, rad, -, rad, rad, rad):
@@ -92,6 +93,13 @@ typedef struct gw_options {      /* NULL => { spin_order 1, isco_cut 0, max_batc
  * right ascension, declination, polarisation angle.                                                     */
 enum { GW_P_MC = 0, GW_P_Q, GW_P_CHI1, GW_P_CHI2, GW_P_DL, GW_P_TC, GW_P_PHIC,
        GW_P_COSI, GW_P_RA, GW_P_DEC, GW_P_PSI, GW_NPARAM = 11 };
+/* A context created with tidal_order > 0 reads GW_NPARAM_TIDAL columns per proposal: the eleven above, then the
+ * dimensionless tidal deformabilities Lambda_1 (of the heavier body, mass m1) and Lambda_2, each finite and >= 0
+ * (else that proposal's outputs are NaN).  The phase gains 3/(128 eta) v^-5 (phi_10 v^10 + phi_12 v^12) with
+ * phi_10 = -sum_A 24 (12 - 11 X_A) X_A^4 Lambda_A, phi_12 = -sum_A (5/28)(3179 - 919 X_A - 2286 X_A^2 +
+ * 260 X_A^3) X_A^4 Lambda_A, X_A = m_A/M (phi_12 only for tidal_order 2).  "theta [n_prop][GW_NPARAM]" below reads
+ * "[n_prop][gw_ctx_n_param(ctx)]" for such a context.                                                      */
+enum { GW_P_LAMBDA1 = 11, GW_P_LAMBDA2 = 12, GW_NPARAM_TIDAL = 13 };
 
 #define GW_MAX_DET 4             /* detectors per context (the fused kernel is specialised per count)    */
 
@@ -153,6 +161,9 @@ int gw_ctx_destroy(gw_ctx *ctx);
 
 /* Introspection.  Any output pointer may be NULL.                                                       */
 int gw_ctx_info(const gw_ctx *ctx, int64_t *n_bins, int *n_det, double *delta_f, int64_t *max_batch);
+
+/* Doubles per theta row this context reads: GW_NPARAM, or GW_NPARAM_TIDAL with the tidal option; -1 for NULL. */
+int gw_ctx_n_param(const gw_ctx *ctx);
 
 /* The launch shape gw_lnl_batch would use for n_prop proposals (what bench.py reports and what fixes
  * the summation order): lanes per proposal, proposals per CTA, number of frequency chunks, CTAs.       */

@@ -23,7 +23,7 @@ GW_OK, GW_ERR_INVALID_ARG, GW_ERR_ALLOC, GW_ERR_CUDA, GW_ERR_ARCH = 0, -1, -2, -
 # every symbol include/gwlnl.h declares (tests/test_abi.py checks the library exports each)
 EXPORTS = (
     "gw_ctx_create", "gw_ctx_reserve", "gw_waveform_batch", "gw_lnl_batch", "gw_lnl_batch_host",
-    "gw_waveform_batch_host", "gw_ctx_destroy", "gw_ctx_info", "gw_ctx_plan", "gw_ctx_norms",
+    "gw_waveform_batch_host", "gw_ctx_destroy", "gw_ctx_info", "gw_ctx_n_param", "gw_ctx_plan", "gw_ctx_norms",
     "gw_ctx_launch_count", "gw_ctx_force_plan", "gw_ctx_kernel_timing", "gw_ctx_last_kernel_ms", "gw_probe_fp64_fma_rate", "gw_strerror", "gw_last_cuda_error", "gw_abi_version",
 )
 
@@ -42,7 +42,7 @@ class gw_detector(ctypes.Structure):
 
 class gw_options(ctypes.Structure):
     _fields_ = [("spin_order", ctypes.c_int), ("isco_cut", ctypes.c_int), ("max_batch", ctypes.c_int64),
-                ("phase_marginal", ctypes.c_int), ("reserved", ctypes.c_int)]
+                ("phase_marginal", ctypes.c_int), ("tidal_order", ctypes.c_int)]
 
 
 def lib_path() -> str:
@@ -74,6 +74,7 @@ def load_library():
     lib.gw_waveform_batch_host.argtypes = [vp, i64, vp, vp, vp]
     lib.gw_ctx_destroy.argtypes = [vp]
     lib.gw_ctx_info.argtypes = [vp, P(i64), P(ci), P(dbl), P(i64)]
+    lib.gw_ctx_n_param.argtypes = [vp]
     lib.gw_ctx_plan.argtypes = [vp, i64, P(ci), P(ci), P(ci), P(i64)]
     lib.gw_ctx_norms.argtypes = [vp, P(dbl)]
     lib.gw_ctx_launch_count.argtypes = [vp]
@@ -134,7 +135,8 @@ class GwContext:
     """
 
     def __init__(self, freqs, data, psd, det_rows, gmst: float, spin_order: int = 1,
-                 max_batch: int = 4096, stream=None, isco_cut: int = 0, phase_marginal: int = 0):
+                 max_batch: int = 4096, stream=None, isco_cut: int = 0, phase_marginal: int = 0,
+                 tidal_order: int = 0):
         self._h = ctypes.c_void_p()
         self._lib = load_library()
         self._keep = []
@@ -145,12 +147,13 @@ class GwContext:
         s_ptr, n_s = self._as_ptr(psd, np.float64)
         if n_d != self.n_det * n_bins or n_s != self.n_det * n_bins:
             raise GwError(GW_ERR_INVALID_ARG, "GwContext", "data/psd must be [n_det][n_bins]")
-        opt = gw_options(int(spin_order), int(isco_cut), int(max_batch), int(phase_marginal), 0)
+        opt = gw_options(int(spin_order), int(isco_cut), int(max_batch), int(phase_marginal), int(tidal_order))
         rc = self._lib.gw_ctx_create(ctypes.byref(self._h), n_bins, f_ptr, self.n_det, d_ptr, s_ptr, dets,
                                      float(gmst), ctypes.byref(opt), _stream_ptr(stream))
         self._keep = []
         _check(rc, "gw_ctx_create")
         self.n_bins = int(n_bins)
+        self.n_param = int(self._lib.gw_ctx_n_param(self._h))     # 11, or 13 with the tidal option
 
     def _as_ptr(self, a, dtype) -> Tuple[int, int]:
         """(pointer, element count in units of dtype) for a numpy array or a torch CUDA tensor."""
@@ -229,12 +232,12 @@ class GwContext:
         _check(self._lib.gw_ctx_reserve(self._h, int(max_batch)), "gw_ctx_reserve", self._h)
 
     # ---- device-pointer entry points ----
-    @staticmethod
-    def _theta_dev(theta):
+    def _theta_dev(self, theta):
         import torch
         if not (isinstance(theta, torch.Tensor) and theta.is_cuda and theta.dtype == torch.float64
-                and theta.is_contiguous() and theta.dim() == 2 and theta.shape[1] == NPARAM):
-            raise GwError(GW_ERR_INVALID_ARG, "theta", "want a contiguous CUDA float64 tensor [n_prop][11]")
+                and theta.is_contiguous() and theta.dim() == 2 and theta.shape[1] == self.n_param):
+            raise GwError(GW_ERR_INVALID_ARG, "theta",
+                          f"want a contiguous CUDA float64 tensor [n_prop][{self.n_param}]")
         return theta
 
     def lnl_batch(self, theta, out=None, parts=None, want_parts: bool = False, stream=None):
@@ -265,7 +268,7 @@ class GwContext:
     # ---- host-buffer entry points (copies inside the call; synchronises) ----
     def lnl_batch_host(self, theta: np.ndarray, out: Optional[np.ndarray] = None,
                        parts: Optional[np.ndarray] = None, want_parts: bool = False, stream=None):
-        th = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, NPARAM)
+        th = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, self.n_param)
         n = th.shape[0]
         if out is None:
             out = np.empty(n)
@@ -277,7 +280,7 @@ class GwContext:
         return (out, parts) if (want_parts or parts is not None) else out
 
     def waveform_batch_host(self, theta: np.ndarray, out: Optional[np.ndarray] = None, stream=None):
-        th = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, NPARAM)
+        th = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1, self.n_param)
         n = th.shape[0]
         if out is None:
             out = np.empty((n, self.n_det, self.n_bins), dtype=np.complex128)

@@ -175,7 +175,7 @@ int reserve_impl(gw_ctx *ctx, int64_t max_batch)
     ok = ok && (e = cudaMalloc(&w.gpartial, sizeof(double) * w.gpartial_doubles)) == cudaSuccess;
     ok = ok && (e = cudaMalloc(&w.gtickets, sizeof(unsigned int) * w.n_gtickets)) == cudaSuccess;
     ok = ok && (e = cudaMemset(w.gtickets, 0, sizeof(unsigned int) * w.n_gtickets)) == cudaSuccess;
-    ok = ok && (e = cudaMalloc(&w.theta_stage, sizeof(double) * max_batch * GW_NPARAM)) == cudaSuccess;
+    ok = ok && (e = cudaMalloc(&w.theta_stage, sizeof(double) * max_batch * ctx->t.n_param)) == cudaSuccess;
     ok = ok && (e = cudaMalloc(&w.lnl_stage, sizeof(double) * max_batch)) == cudaSuccess;
     ok = ok && (e = cudaMalloc(&w.parts_stage, sizeof(double) * max_batch * n_det * 3)) == cudaSuccess;
     ok = ok && (e = cudaMemset(w.tickets, 0, sizeof(unsigned int) * w.n_tickets)) == cudaSuccess;
@@ -250,7 +250,7 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
     gw_options o = {1, 0, 4096, 0, 0};
     if (opt) o = *opt;
     if (o.spin_order < 0 || o.spin_order > 1 || o.isco_cut < 0 || o.isco_cut > 1 || o.max_batch < 1 ||
-        o.phase_marginal < 0 || o.phase_marginal > 1 || o.reserved != 0)
+        o.phase_marginal < 0 || o.phase_marginal > 1 || o.tidal_order < 0 || o.tidal_order > 2)
         return GW_ERR_INVALID_ARG;
 
     cudaStream_t s = (cudaStream_t)cuda_stream;
@@ -319,6 +319,7 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
     Tables &t = ctx->t;
     t.n_bins = n_bins; t.n_pad = (n_bins + 31) / 32 * 32 + 32; t.n_det = n_det; t.f0 = f0; t.delta_f = df;
     t.isco_cut = o.isco_cut; t.phase_marginal = o.phase_marginal;
+    t.tidal_order = o.tidal_order; t.n_param = o.tidal_order > 0 ? (int)GW_NPARAM_TIDAL : (int)GW_NPARAM;
     do {
         if ((e = configure_kernels(nullptr)) != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
         ctx->ctas_per_sm = fused_ctas_per_sm(n_det);
@@ -378,6 +379,8 @@ int gw_ctx_info(const gw_ctx *ctx, int64_t *n_bins, int *n_det, double *delta_f,
     if (max_batch) *max_batch = ctx->w.max_batch;
     return GW_OK;
 }
+
+int gw_ctx_n_param(const gw_ctx *ctx) { return ctx ? ctx->t.n_param : -1; }
 
 int gw_ctx_plan(const gw_ctx *ctx, int64_t n_prop, int *lanes_per_prop, int *props_per_cta, int *n_chunks,
                 int64_t *n_ctas)
@@ -486,7 +489,7 @@ int gw_lnl_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, dou
     DeviceGuard guard(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     Workspace &w = ctx->w;
-    cudaError_t e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * GW_NPARAM,
+    cudaError_t e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * ctx->t.n_param,
                                     cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     // lnL goes straight to a pinned output buffer (coalesced 8-byte stores of the finish stage over the host link):
@@ -528,11 +531,11 @@ int gw_waveform_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host
         w.h_stage_doubles = want;
     }
     const int64_t slab = w.h_stage_doubles / per_prop;
-    e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * GW_NPARAM, cudaMemcpyHostToDevice, s);
+    e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * ctx->t.n_param, cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     for (int64_t b0 = 0; b0 < n_prop; b0 += slab) {
         const int64_t nb = (n_prop - b0 < slab) ? n_prop - b0 : slab;
-        rc = gw_waveform_batch(ctx, nb, w.theta_stage + b0 * GW_NPARAM, w.h_stage, cuda_stream);
+        rc = gw_waveform_batch(ctx, nb, w.theta_stage + b0 * ctx->t.n_param, w.h_stage, cuda_stream);
         if (rc != GW_OK) return rc;
         e = cudaMemcpyAsync(h_out_host + b0 * per_prop, w.h_stage, sizeof(double) * nb * per_prop,
                             cudaMemcpyDeviceToHost, s);

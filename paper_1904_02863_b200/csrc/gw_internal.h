@@ -40,10 +40,12 @@ constexpr int kExclusiveSmemBytes = 120 * 1024;   // > half of an SM's 228 KB: a
 constexpr int kRecFixed   = 10;    // record fields before the per-detector block
 constexpr int kRecPerDet  = 5;     // tau, Cre, Cim, rot_re, rot_im
 // record fields: 0..8 phase coefficients, then kRecPerDet per detector, then f_ISCO and the index of the last
-// bin with f_j <= f_ISCO (as a double)
+// bin with f_j <= f_ISCO (as a double), then the two tidal coefficients (of x^5 and x^7; zero without the option)
 __host__ __device__ constexpr int rec_field_fisco(int n_det) { return 9 + kRecPerDet * n_det; }
 __host__ __device__ constexpr int rec_field_jcut(int n_det)  { return 10 + kRecPerDet * n_det; }
-__host__ __device__ constexpr int rec_fields(int n_det)      { return 11 + kRecPerDet * n_det; }
+__host__ __device__ constexpr int rec_field_t10(int n_det)   { return 11 + kRecPerDet * n_det; }
+__host__ __device__ constexpr int rec_field_t12(int n_det)   { return 12 + kRecPerDet * n_det; }
+__host__ __device__ constexpr int rec_fields(int n_det)      { return 13 + kRecPerDet * n_det; }
 
 // One detector as the kernels see it (built on the host from gw_detector).
 struct DetGeom {
@@ -64,6 +66,8 @@ struct Tables {
     double  i7[GW_MAX_DET];   // host copy of I7_I = sum_j (4 df/S_Ij) f_j^(-7/3)
     double *i7cum;        // isco_cut only: [n_det][n_pad] inclusive prefix sums of (4 df/S_Ij) f_j^(-7/3)
     int     isco_cut, phase_marginal;
+    int     tidal_order;  // 0 | 1 (5PN) | 2 (5PN + 6PN): NEXT-1 option
+    int     n_param;      // doubles per theta row: GW_NPARAM, or GW_NPARAM_TIDAL with the tidal option
 };
 
 // Launch shape of one gw_lnl_batch call (a pure function of n_prop and the context; fixes summation order).
@@ -88,7 +92,7 @@ struct Workspace {
     int64_t gpartial_doubles;
     unsigned int *gtickets;
     int64_t n_gtickets;
-    double *theta_stage;  // [max_batch][GW_NPARAM]   (host-variant staging)
+    double *theta_stage;  // [max_batch][n_param]     (host-variant staging)
     double *lnl_stage;    // [max_batch]
     double *parts_stage;  // [max_batch][n_det][3]
     double *h_stage;      // waveform slab staging (host variant), h_stage_doubles

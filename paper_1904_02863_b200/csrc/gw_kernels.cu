@@ -149,6 +149,7 @@ struct SetupArgs {
     DetSet  dets;
     double  gmst;
     int     n_det, spin_order;
+    int     n_param, tidal_order;   // doubles per theta row; NEXT-1 tidal option (0 | 1 | 2)
     int64_t n_prop, rec_stride;
     const double *theta;
     double *rec;
@@ -170,7 +171,7 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
     const int role = threadIdx.x >> 5;
     const int64_t b = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
     if (b >= a.n_prop) return;
-    const double *th = a.theta + b * GW_NPARAM;
+    const double *th = a.theta + b * a.n_param;
     double *r = a.rec + b;
     const int64_t S = a.rec_stride;
     const double mc = th[GW_P_MC];
@@ -219,6 +220,29 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
         r[6 * S] = kPhaseScale * (pref * kap * (phi6 + ph6l * lnk));                                // c6  * x
         r[7 * S] = kPhaseScale * (pref * kap * ph6l / 3.0);                                         // cL6 * x ln f
         r[8 * S] = kPhaseScale * (pref * kap * kap * phi7);                                         // c7  * x^2
+        // NEXT-1 option tidal_order: 5PN and 6PN adiabatic tidal terms in the per-body coding,
+        //   phi_10 = -sum_A 24 (12 - 11 X_A) X_A^4 Lambda_A,
+        //   phi_12 = -sum_A (5/28)(3179 - 919 X_A - 2286 X_A^2 + 260 X_A^3) X_A^4 Lambda_A,   X_A = m_A / M,
+        // as coefficients of x^5 and x^7 (v = kappa x).  Lambda_A must be finite and >= 0.
+        double t10 = 0.0, t12 = 0.0;
+        bool tidal_ok = true;
+        if (a.tidal_order >= 1) {
+            const double lam[2] = {th[GW_P_LAMBDA1], th[GW_P_LAMBDA2]};
+            const double X[2]   = {1.0 / opq, q / opq};
+            double p10 = 0.0, p12 = 0.0;
+#pragma unroll
+            for (int A = 0; A < 2; ++A) {
+                const double x = X[A], x2 = x * x, w = x2 * x2 * lam[A];
+                p10 -= 24.0 * (12.0 - 11.0 * x) * w;
+                p12 -= (5.0 / 28.0) * (3179.0 + x * (-919.0 + x * (-2286.0 + x * 260.0))) * w;
+                tidal_ok = tidal_ok && (lam[A] >= 0.0) && isfinite(lam[A]);
+            }
+            const double k2 = kap * kap, k5 = k2 * k2 * kap;
+            t10 = kPhaseScale * (pref * p10 * k5);                                                  // t10 * x^5
+            if (a.tidal_order >= 2) t12 = kPhaseScale * (pref * p12 * k5 * k2);                     // t12 * x^7
+        }
+        r[(int64_t)rec_field_t10(a.n_det) * S] = t10;
+        r[(int64_t)rec_field_t12(a.n_det) * S] = t12;
         {   // domain of the integer range reduction (cis_quarter_turns: |phase| < 2^31 quarter turns): bound the
             // phase over the band by its terms at the band edges; beyond 1e9 phase units the proposal is poisoned
             const double x0 = cbrt(a.f0), xi = 1.0 / x0, x1 = cbrt(a.f_max), tc = th[GW_P_TC];
@@ -226,8 +250,9 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
             const double bound = fabs(r[0 * S]) * (xi * xi) * (xi * xi) * xi + fabs(r[1 * S]) * (xi * xi * xi) +
                                  fabs(r[2 * S]) * (xi * xi) + fabs(r[3 * S]) * xi + fabs(r[4 * S]) +
                                  fabs(r[5 * S]) * l1 + fabs(r[6 * S]) * x1 + fabs(r[7 * S]) * x1 * l1 +
-                                 fabs(r[8 * S]) * x1 * x1 + kPhaseScale * (fabs(tc) + 1.0) * a.f_max;
-            if (!(bound < 1.0e9)) r[4 * S] = __longlong_as_double(0x7ff8000000000000LL);
+                                 fabs(r[8 * S]) * x1 * x1 + kPhaseScale * (fabs(tc) + 1.0) * a.f_max +
+                                 (fabs(t10) + fabs(t12) * x1 * x1) * (x1 * x1) * (x1 * x1) * x1;
+            if (!(bound < 1.0e9) || !tidal_ok) r[4 * S] = __longlong_as_double(0x7ff8000000000000LL);
         }
         // NEXT-1 option isco_cut: f_ISCO = 1/(6^(3/2) pi M) and the last bin with f_j <= f_ISCO (-1: none).
         // The decision is taken in fp64 against the same f_j the oracle compares with.
@@ -308,6 +333,7 @@ cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int s
 {
     SetupArgs a;
     a.dets = dets; a.gmst = gmst; a.n_det = t.n_det; a.spin_order = spin_order;
+    a.n_param = t.n_param; a.tidal_order = t.tidal_order;
     a.n_prop = n_prop; a.rec_stride = rec_stride; a.theta = theta_dev; a.rec = rec;
     a.rot_stride_hz = rot_stride_hz; a.relative_tau = relative_tau;
     a.f_amp = reinterpret_cast<const double2 *>(t.planes) + 4 * t.n_pad;
@@ -372,10 +398,11 @@ struct WaveArgs {
     double *h;
 };
 
-template <int NDET>
+template <int NDET, bool TIDAL>
 __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(const WaveArgs a)
 {
-    constexpr int NF = 10 + 4 * NDET;            // doubles per staged record: 9 coefs + pad, (tau, pad, CAre, CAim) per det
+    constexpr int NT = 10 + 4 * NDET;            // index of the tidal pair (t10, t12) of a staged record
+    constexpr int NF = NT + (TIDAL ? 2 : 0);     // doubles per staged record: 9 coefs + f_ISCO, (tau, pad, CAre, CAim) per det
     __shared__ __align__(16) double srec[kWfProps][NF];
     const int     tid     = threadIdx.x;
     const int     bin_blk = blockIdx.x % a.bin_blocks;
@@ -383,6 +410,7 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
     const double2 *pl = reinterpret_cast<const double2 *>(a.planes);
     double2 b01[kWfBins], b23[kWfBins], b45[kWfBins], b67[kWfBins];
     double  amp[kWfBins], f[kWfBins];
+    double  x5[kWfBins], x7[kWfBins];            // TIDAL: x^5, x^7 of the thread's bins (x = f^(1/3))
     int64_t j[kWfBins];
     bool    in[kWfBins];
 #pragma unroll
@@ -394,6 +422,11 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
         b45[u] = pl[2 * a.n_pad + jc]; b67[u] = pl[3 * a.n_pad + jc];
         const double2 fa = pl[4 * a.n_pad + jc];
         f[u] = fa.x; amp[u] = fa.y;
+        if (TIDAL) {
+            const double x2 = b67[u].y;
+            x5[u] = (x2 * x2) * b45[u].y;
+            x7[u] = x5[u] * x2;
+        }
     }
     pdl_wait_primary();                          // the records come from the setup kernel
     const int64_t b0 = p_blk * kWfProps;
@@ -403,6 +436,7 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
         double v = 0.0;
         if (fld < 9) v = a.rec[(int64_t)fld * a.rec_stride + b0 + p];
         else if (fld == 9) v = a.isco_cut ? a.rec[(int64_t)rec_field_fisco(NDET) * a.rec_stride + b0 + p] : 1.0e308;
+        else if (TIDAL && fld >= NT) v = a.rec[(int64_t)(rec_field_t10(NDET) + (fld - NT)) * a.rec_stride + b0 + p];
         else {
             const int i = (fld - 10) >> 2, w = (fld - 10) & 3;          // w: 0 tau, 2 CAre, 3 CAim
             if (w != 1) v = a.rec[(int64_t)(9 + kRecPerDet * i + (w == 0 ? 0 : w - 1)) * a.rec_stride + b0 + p];
@@ -420,6 +454,11 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
         double ph[kWfBins];
 #pragma unroll
         for (int u = 0; u < kWfBins; ++u) ph[u] = phase_turns(k, b01[u], b23[u], b45[u], b67[u]);
+        if (TIDAL) {                                                     // NEXT-1 option: + t10 x^5 + t12 x^7
+            const double2 tt = r2[NT / 2];
+#pragma unroll
+            for (int u = 0; u < kWfBins; ++u) ph[u] = __fma_rn(tt.y, x7[u], __fma_rn(tt.x, x5[u], ph[u]));
+        }
         const double f_cut = k8.y;                                       // f_ISCO, or 1e308 without the cut-off
         double2 *row = h + ((b0 + p) * NDET) * a.n_bins;
 #pragma unroll
@@ -440,7 +479,7 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
     }
 }
 
-template <int NDET>
+template <int NDET, bool TIDAL>
 static cudaError_t launch_waveform_t(const WaveArgs &a, int64_t blocks, cudaStream_t s)
 {
     cudaLaunchConfig_t cfg = {};
@@ -449,7 +488,7 @@ static cudaError_t launch_waveform_t(const WaveArgs &a, int64_t blocks, cudaStre
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, waveform_kernel<NDET>, a);
+    return cudaLaunchKernelEx(&cfg, waveform_kernel<NDET, TIDAL>, a);
 }
 
 cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, int64_t rec_stride,
@@ -465,11 +504,12 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
     const int64_t blocks = p_blocks * a.bin_blocks;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     *launches += 1;
+    const bool tidal = t.tidal_order > 0;
     switch (t.n_det) {
-    case 1: return launch_waveform_t<1>(a, blocks, s);
-    case 2: return launch_waveform_t<2>(a, blocks, s);
-    case 3: return launch_waveform_t<3>(a, blocks, s);
-    case 4: return launch_waveform_t<4>(a, blocks, s);
+    case 1: return tidal ? launch_waveform_t<1, true>(a, blocks, s) : launch_waveform_t<1, false>(a, blocks, s);
+    case 2: return tidal ? launch_waveform_t<2, true>(a, blocks, s) : launch_waveform_t<2, false>(a, blocks, s);
+    case 3: return tidal ? launch_waveform_t<3, true>(a, blocks, s) : launch_waveform_t<3, false>(a, blocks, s);
+    case 4: return tidal ? launch_waveform_t<4, true>(a, blocks, s) : launch_waveform_t<4, false>(a, blocks, s);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -544,7 +584,7 @@ __device__ __forceinline__ void finish_proposal(const FusedArgs &a, int64_t b, c
     a.lnl[b] = lnl;
 }
 
-template <int NDET, bool MULTI, bool ISCO>
+template <int NDET, bool MULTI, bool ISCO, bool TIDAL>
 __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedArgs a)
 {
     constexpr int NP = kBasisPlanes + NDET;                  // planes per stage
@@ -593,6 +633,11 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
 
     pdl_wait_primary();                                      // records come from the setup kernel
     const PhaseCoef k = load_coef(a.rec, a.rec_stride, b);
+    double t10 = 0.0, t12 = 0.0;                             // NEXT-1 option: tidal terms t10 x^5 + t12 x^7
+    if (TIDAL) {
+        t10 = a.rec[(int64_t)rec_field_t10(NDET) * a.rec_stride + b];
+        t12 = a.rec[(int64_t)rec_field_t12(NDET) * a.rec_stride + b];
+    }
     double tau[NDET], rr[NDET], ri_[NDET], zr[NDET], zi[NDET];
 #pragma unroll
     for (int i = 0; i < NDET; ++i) {
@@ -660,12 +705,28 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                     for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.cL5, v[u].x, ph[u]);
 #pragma unroll
                     for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.c6, v[u].y, ph[u]);
+                    double x1[kUnroll];                              // TIDAL: x = f^(1/3) of the bins
+                    if (TIDAL) {
+#pragma unroll
+                        for (int u = 0; u < kUnroll; ++u) x1[u] = v[u].y;
+                    }
 #pragma unroll
                     for (int u = 0; u < kUnroll; ++u) v[u] = P[3 * kStageBins + it + u];
 #pragma unroll
                     for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.cL6, v[u].x, ph[u]);
 #pragma unroll
                     for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(k.c7, v[u].y, ph[u]);
+                    if (TIDAL) {                                     // + x^5 (t10 + t12 x^2): 4 more fp64 instructions
+                        double x5[kUnroll], tt[kUnroll];
+#pragma unroll
+                        for (int u = 0; u < kUnroll; ++u) x5[u] = v[u].y * v[u].y;
+#pragma unroll
+                        for (int u = 0; u < kUnroll; ++u) tt[u] = __fma_rn(t12, v[u].y, t10);
+#pragma unroll
+                        for (int u = 0; u < kUnroll; ++u) x5[u] *= x1[u];
+#pragma unroll
+                        for (int u = 0; u < kUnroll; ++u) ph[u] = __fma_rn(tt[u], x5[u], ph[u]);
+                    }
 #pragma unroll
                     for (int u = 0; u < kUnroll; ++u) v[u] = P[4 * kStageBins + it + u];
 #pragma unroll
@@ -733,6 +794,10 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             if (MULTI) { masked = jj >= cnt; jj = masked ? cnt - 1 : jj; }
             double ph = phase_turns(k, P[0 * kStageBins + jj], P[1 * kStageBins + jj],
                                     P[2 * kStageBins + jj], P[3 * kStageBins + jj]);
+            if (TIDAL) {
+                const double x = P[2 * kStageBins + jj].y, x2 = P[3 * kStageBins + jj].y;
+                ph = __fma_rn(__fma_rn(t12, x2, t10), (x2 * x2) * x, ph);
+            }
             ph = __fma_rn(tau[0], P[4 * kStageBins + jj].x, ph);
             double c, sn;
             cis_phase_lnl(ph, c, sn);
@@ -914,7 +979,7 @@ size_t fused_smem_bytes_exclusive(int n_det)
     return need > half ? need : half;
 }
 
-template <int NDET, bool MULTI, bool ISCO>
+template <int NDET, bool MULTI, bool ISCO, bool TIDAL>
 static cudaError_t launch_fused_t(const FusedArgs &a, int64_t blocks, bool exclusive, cudaStream_t s)
 {
     cudaLaunchConfig_t cfg = {};
@@ -924,7 +989,7 @@ static cudaError_t launch_fused_t(const FusedArgs &a, int64_t blocks, bool exclu
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, fused_kernel<NDET, MULTI, ISCO>, a);
+    return cudaLaunchKernelEx(&cfg, fused_kernel<NDET, MULTI, ISCO, TIDAL>, a);
 }
 
 cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, const double *rec,
@@ -941,14 +1006,18 @@ cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, cons
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     *launches += 1;
     a.i7cum = t.i7cum; a.phase_marginal = t.phase_marginal;
-    const int variant = (plan.lpp > 1 ? 1 : 0) + (t.isco_cut ? 2 : 0);
+    const int variant = (plan.lpp > 1 ? 1 : 0) + (t.isco_cut ? 2 : 0) + (t.tidal_order > 0 ? 4 : 0);
     const bool ex = plan.exclusive != 0;
 #define GW_DISPATCH(N)                                                                      \
     switch (variant) {                                                                      \
-    case 0: return launch_fused_t<N, false, false>(a, blocks, ex, s);                           \
-    case 1: return launch_fused_t<N, true, false>(a, blocks, ex, s) ;                            \
-    case 2: return launch_fused_t<N, false, true>(a, blocks, ex, s) ;                            \
-    default: return launch_fused_t<N, true, true>(a, blocks, ex, s);                            \
+    case 0: return launch_fused_t<N, false, false, false>(a, blocks, ex, s);                \
+    case 1: return launch_fused_t<N, true, false, false>(a, blocks, ex, s);                 \
+    case 2: return launch_fused_t<N, false, true, false>(a, blocks, ex, s);                 \
+    case 3: return launch_fused_t<N, true, true, false>(a, blocks, ex, s);                  \
+    case 4: return launch_fused_t<N, false, false, true>(a, blocks, ex, s);                 \
+    case 5: return launch_fused_t<N, true, false, true>(a, blocks, ex, s);                  \
+    case 6: return launch_fused_t<N, false, true, true>(a, blocks, ex, s);                  \
+    default: return launch_fused_t<N, true, true, true>(a, blocks, ex, s);                  \
     }
     switch (t.n_det) {
     case 1: GW_DISPATCH(1)
@@ -967,16 +1036,17 @@ static cudaError_t configure_one()
 {
     const int smem = (int)fused_smem_bytes_exclusive(NDET);
     cudaError_t e;
-    e = cudaFuncSetAttribute(fused_kernel<NDET, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(fused_kernel<NDET, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(fused_kernel<NDET, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(fused_kernel<NDET, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
+    const void *variants[8] = {
+        (const void *)fused_kernel<NDET, false, false, false>, (const void *)fused_kernel<NDET, true, false, false>,
+        (const void *)fused_kernel<NDET, false, true, false>,  (const void *)fused_kernel<NDET, true, true, false>,
+        (const void *)fused_kernel<NDET, false, false, true>,  (const void *)fused_kernel<NDET, true, false, true>,
+        (const void *)fused_kernel<NDET, false, true, true>,   (const void *)fused_kernel<NDET, true, true, true>};
+    for (int v = 0; v < 8; ++v) {
+        e = cudaFuncSetAttribute(variants[v], cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+    }
     int n = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fused_kernel<NDET, false, false>, kThreads, fused_smem_bytes(NDET));
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fused_kernel<NDET, false, false, false>, kThreads, fused_smem_bytes(NDET));
     if (e != cudaSuccess) return e;
     g_ctas_per_sm[NDET] = n > 0 ? n : 1;
     return cudaSuccess;

@@ -34,10 +34,11 @@ def test_header_symbols_are_exported(lib):
 
 
 def test_no_compute_calls(lib):
-    assert lib.gw_abi_version() == 2
+    assert lib.gw_abi_version() == 3
     assert lib.gw_strerror(0) == b"ok" and b"invalid" in lib.gw_strerror(-1)
     assert lib.gw_ctx_destroy(None) == 0
     assert lib.gw_ctx_info(None, None, None, None, None) == -1
+    assert lib.gw_ctx_n_param(None) == -1
     assert lib.gw_lnl_batch(None, 1, None, None, None, None) == -1
     assert lib.gw_waveform_batch(None, 1, None, None, None) == -1
     assert lib.gw_ctx_reserve(None, 8) == -1
