@@ -78,3 +78,28 @@ def test_waveform_full_size(oracle, name, batch, n_sample):
     h_ref = oracle.waveform(f, dets, cfg.gmst, th[idx], cfg.spin_order)
     worst = assert_h_close(h_gpu, h_ref)
     print(f"{name} B={batch} sampled={len(idx)} worst |dh|/max|h| = {worst:.2e}")
+
+
+@pytest.mark.parametrize("name,batch,n_sample", [("C2", 1024, 6), ("C3", 256, 3)], ids=["C2-tidal", "C3-tidal"])
+def test_lnl_full_size_tidal(oracle, name, batch, n_sample):
+    """The neutron-star workloads at full size with the tidal option (NEXT-1; 13-column theta, TIDAL kernel variant),
+    same data as above (a point-mass injection), sampled proposals against the oracle + run-to-run identical bits."""
+    import torch
+    from paper_1904_02863_b200 import GwContext
+    cfg = inputs.CONFIGS[name]
+    f, S, dets, d, th_all = _problem(oracle, name)
+    th, lam = th_all[:batch], inputs.tidal_lambdas(cfg, batch)
+    th13 = np.ascontiguousarray(np.hstack([th, lam]))
+    with GwContext(f, d, S, dets, cfg.gmst, spin_order=cfg.spin_order, max_batch=batch, tidal_order=2) as ctx:
+        thd = torch.from_numpy(th13).cuda()
+        lnl, parts = ctx.lnl_batch(thd, want_parts=True)
+        lnl2, parts2 = ctx.lnl_batch(thd, want_parts=True)
+        torch.cuda.synchronize()
+        assert torch.equal(lnl, lnl2) and torch.equal(parts, parts2)
+        lnl, parts = lnl.cpu().numpy(), parts.cpu().numpy()
+    assert np.all(np.isfinite(lnl)) and np.all(parts[..., 2] > 0)
+    idx = _sample(batch, n_sample, 3000 + batch)
+    lnl_ref, parts_ref, _ = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[idx], cfg.spin_order,
+                                       lambdas=lam[idx], tidal_order=2)
+    worst = assert_lnl_close(lnl[idx], parts[idx], lnl_ref, parts_ref)
+    print(f"{name} tidal B={batch} sampled={len(idx)} worst_rel={worst:.2e}")
