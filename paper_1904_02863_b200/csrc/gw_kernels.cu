@@ -375,7 +375,7 @@ __device__ __forceinline__ double phase_turns(const PhaseCoef &k, double2 b01, d
 // =====================================================================================================
 // K2: waveform-only kernel (north_star item (3); step a6).  Lanes run along bins so that every store is
 // a 16-byte element of a 512-byte contiguous warp segment; each thread keeps its bin's basis in
-// registers and walks kPropsPerCta proposals, so table reads are amortised and HBM traffic is the
+// registers and walks props_per_cta proposals, so table reads are amortised and HBM traffic is the
 // 16 B/element store stream.
 //     h_I(f) = CA_I f^(-7/6) exp(-2 pi i (Phi'(f) + f tau_I))
 // =====================================================================================================
@@ -388,13 +388,17 @@ __device__ __forceinline__ double phase_turns(const PhaseCoef &k, double2 b01, d
 #ifndef GW_WF_MIN_CTAS
 #define GW_WF_MIN_CTAS 1
 #endif
-constexpr int kWfProps = GW_WF_PROPS;     // proposals per CTA
+constexpr int kWfProps = GW_WF_PROPS;     // proposals per CTA while the five basis planes stay L2-resident
+constexpr int kWfPropsLong = 64;          // ... and for long signals, whose planes stream from HBM once per proposal
+                                          // block: 80 B of table reads per bin against 48 N_det B stored per proposal
+constexpr int64_t kWfLongBins = 400000;   // 5 planes x 16 B x 400k bins = 32 MB: beyond this the planes do not stay in L2
 constexpr int kWfBins  = GW_WF_BINS;      // bins per thread (kThreads * kWfBins bins per CTA)
 
 struct WaveArgs {
     const double *planes, *rec;
     int64_t n_pad, n_bins, n_prop, rec_stride;
     int     bin_blocks, isco_cut;
+    int     props_per_cta;   // kWfProps | kWfPropsLong
     double *h;
 };
 
@@ -403,7 +407,7 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
 {
     constexpr int NT = 10 + 4 * NDET;            // index of the tidal pair (t10, t12) of a staged record
     constexpr int NF = NT + (TIDAL ? 2 : 0);     // doubles per staged record: 9 coefs + f_ISCO, (tau, pad, CAre, CAim) per det
-    __shared__ __align__(16) double srec[kWfProps][NF];
+    __shared__ __align__(16) double srec[kWfPropsLong][NF];
     const int     tid     = threadIdx.x;
     const int     bin_blk = blockIdx.x % a.bin_blocks;
     const int64_t p_blk   = blockIdx.x / a.bin_blocks;
@@ -429,8 +433,8 @@ __global__ void __launch_bounds__(kThreads, GW_WF_MIN_CTAS) waveform_kernel(cons
         }
     }
     pdl_wait_primary();                          // the records come from the setup kernel
-    const int64_t b0 = p_blk * kWfProps;
-    const int     np = (int)((b0 + kWfProps < a.n_prop) ? kWfProps : a.n_prop - b0);
+    const int64_t b0 = p_blk * a.props_per_cta;
+    const int     np = (int)((b0 + a.props_per_cta < a.n_prop) ? a.props_per_cta : a.n_prop - b0);
     for (int idx = tid; idx < np * NF; idx += kThreads) {
         const int p = idx / NF, fld = idx % NF;
         double v = 0.0;
@@ -500,7 +504,8 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
     a.bin_blocks = (int)((t.n_bins + kThreads * kWfBins - 1) / (kThreads * kWfBins));
     a.isco_cut = t.isco_cut;
     a.h = h_out;
-    const int64_t p_blocks = (n_prop + kWfProps - 1) / kWfProps;
+    a.props_per_cta = t.n_bins > kWfLongBins ? kWfPropsLong : kWfProps;
+    const int64_t p_blocks = (n_prop + a.props_per_cta - 1) / a.props_per_cta;
     const int64_t blocks = p_blocks * a.bin_blocks;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     *launches += 1;
