@@ -331,7 +331,7 @@ def test_time_shift_interchange(oracle, torch_cuda):
 @pytest.mark.parametrize("seed", range(int(os.environ.get("GW_RANDOM_SHAPES", "24"))))   # soak: GW_RANDOM_SHAPES=500
 def test_random_shapes(oracle, torch_cuda, seed):
     """Seeded random shapes: bins 2..2500, proposals 1..700, 1..4 detectors (geometric and fixed mixed), random band,
-    resolution, mass range and options -- ragged tails everywhere the launch planner can put one."""
+    resolution, mass range and options (incl. the tidal orders) -- ragged tails everywhere the launch planner can put one."""
     torch = torch_cuda
     from paper_1904_02863_b200 import GwContext, GwError
     rng = np.random.Generator(np.random.PCG64(4242 + seed))
@@ -368,8 +368,13 @@ def test_random_shapes(oracle, torch_cuda, seed):
     z = rng.standard_normal((n_det, M, 2))
     d = oracle.waveform(f, dets, gmst, th[:1], spin)[0] + (z[..., 0] + 1j * z[..., 1]) * np.sqrt(S / (4 * df))
     rng2 = np.random.Generator(np.random.PCG64(777 + seed))          # every other case: a pinned launch shape
-    with GwContext(f, d, S, dets, gmst, spin_order=spin, max_batch=B, isco_cut=isco, phase_marginal=marg) as ctx:
-        thd = _dev(torch, th)
+    rng3 = np.random.Generator(np.random.PCG64(999 + seed))          # one case in three each: tidal order 0, 1, 2
+    tidal = int(rng3.integers(0, 3))
+    lam = rng3.uniform(0, 5000, (B, 2))
+    tkw = dict(lambdas=lam, tidal_order=tidal) if tidal else {}
+    with GwContext(f, d, S, dets, gmst, spin_order=spin, max_batch=B, isco_cut=isco, phase_marginal=marg,
+                   tidal_order=tidal) as ctx:
+        thd = _dev(torch, np.hstack([th, lam]) if tidal else th)
         if rng2.random() < 0.5:
             lpp = int(rng2.choice([1, 2, 4, 8, 16, 32]))
             ctx.force_plan(lpp, int(rng2.integers(1, max(2, min(80, M // lpp + 1)))))
@@ -383,7 +388,7 @@ def test_random_shapes(oracle, torch_cuda, seed):
         h = ctx.waveform_batch(thd[: min(B, 16)].contiguous())
         torch.cuda.synchronize()
         lnl, parts, h = lnl.cpu().numpy(), parts.cpu().numpy(), h.cpu().numpy()
-    lnl_ref, parts_ref, _ = oracle.lnl(f, df, d, S, dets, gmst, th, spin, isco_cut=isco)
+    lnl_ref, parts_ref, _ = oracle.lnl(f, df, d, S, dets, gmst, th, spin, isco_cut=isco, **tkw)
     if marg:
         lnl_ref = oracle.lnl_phase_marginal(parts_ref)
     hh = parts_ref[..., 2].sum(axis=1)
@@ -400,7 +405,9 @@ def test_random_shapes(oracle, torch_cuda, seed):
         pscale = (np.hypot(parts_ref[keep][..., 0], parts_ref[keep][..., 1]) + parts_ref[keep][..., 2])[..., None]
         ok = pscale[..., 0] > 0
         assert (np.abs(parts[keep] - parts_ref[keep])[ok] / pscale[ok]).max() <= 1e-8
-    h_ref = oracle.waveform(f, dets, gmst, th[: min(B, 16)], spin, isco_cut=isco)
+    if tidal:
+        tkw["lambdas"] = lam[: min(B, 16)]
+    h_ref = oracle.waveform(f, dets, gmst, th[: min(B, 16)], spin, isco_cut=isco, **tkw)
     hs = np.abs(h_ref).max(axis=-1, keepdims=True)
     nz = hs[..., 0] > 0
     assert np.all(h[~nz] == 0)
