@@ -246,3 +246,32 @@ def test_call_sequences_leave_no_state_behind(oracle, seed):
             assert np.array_equal(g[0], want[0]) and np.array_equal(g[1], want[1]), c
             n_checked += 1
     assert n_checked >= 20
+
+
+def test_tidal_outputs_stay_inside_their_buffers_and_theta_is_read_with_its_stride(oracle):
+    """Guard bands around the outputs of the TIDAL kernel variants, and theta [B][13] placed at the very end of its
+    allocation's used range with a NaN canary after it: a read with the wrong stride or past the last row would
+    poison a result.  After a reserve() growth the 13-column host staging still holds the whole batch."""
+    import torch
+    from paper_1904_02863_b200 import GwContext
+    cfg = inputs.CONFIGS["C2"].reduced(f_max=60.0, duration_s=4.0, batch=600)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    lam = inputs.tidal_lambdas(cfg)
+    th13 = np.ascontiguousarray(np.hstack([th, lam]))
+    with GwContext(f, d, S, dets, cfg.gmst, spin_order=cfg.spin_order, max_batch=64, tidal_order=2) as ctx:
+        ctx.reserve(600)
+        ref_host = ctx.lnl_batch_host(th13)
+        for B in (1, 5, 33, 256, 257, 600):
+            tbuf = torch.full((B * 13 + GUARD,), float("nan"), dtype=torch.float64, device="cuda")
+            tbuf[:B * 13] = torch.from_numpy(th13[:B].ravel()).cuda()
+            thd = tbuf[:B * 13].view(B, 13)
+            nl, npart, nh = B, B * cfg.n_det * 3, B * cfg.n_det * cfg.n_bins * 2
+            lbuf, lnl = _guarded(torch, nl)
+            pbuf, parts = _guarded(torch, npart)
+            hbuf, h = _guarded(torch, nh)
+            ctx.lnl_batch(thd, out=lnl, parts=parts.view(B, cfg.n_det, 3))
+            ctx.waveform_batch(thd, out=torch.view_as_complex(h.view(B, cfg.n_det, cfg.n_bins, 2)))
+            torch.cuda.synchronize()
+            assert _intact(torch, lbuf, nl) and _intact(torch, pbuf, npart) and _intact(torch, hbuf, nh), B
+            assert bool(torch.isfinite(lnl).all()) and bool(torch.isfinite(parts).all()) and bool(torch.isfinite(h).all()), B
+        assert np.array_equal(ref_host, lnl.cpu().numpy())          # B = 600: host variant == device variant
