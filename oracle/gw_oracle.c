@@ -37,7 +37,9 @@
  * closed-form special case (P5), light-travel-time bounds (P6), 40-digit
  * mpmath spot values (P7), a hand-expanded tiny case (P8), bin independence
  * (P9); the tidal option (NEXT-1): Lambda~ form against the per-body form, re-derivation from the tidal
- * energy and flux, equal-mass special case, 40-digit spot values (P10, tests/test_oracle_tidal.py).
+ * energy and flux, equal-mass special case, 40-digit spot values (P10, tests/test_oracle_tidal.py); spin_order 2:
+ * re-derivation of the 2.5/3/3.5PN spin-orbit terms from the spin-orbit energy and flux, (chi_s, chi_a) coding,
+ * special cases (P11, tests/test_oracle_spin35.py).
  * The digits of the H1/L1/V1 geometry are input data, not oracle
  * arithmetic; they are pinned by invariants only.
  */
@@ -88,7 +90,16 @@ void gwo_masses(double mc_msun, double q, double *eta, double *mtot_s, double *m
 
 /* ---- O2: TaylorF2 phase coefficients (readings A5, A7, A8) ---- */
 /* phi[k] multiplies v^k, phil[k] multiplies v^k ln v, k = 0..7; phi[1] = 0.
- * spin_order 0: beta = sigma = 0;  1: 1.5PN spin-orbit beta and 2PN spin-spin sigma.        */
+ * spin_order 0: beta = sigma = 0;  1: 1.5PN spin-orbit beta and 2PN spin-spin sigma;
+ * 2 (NEXT-1 option, reading A22): in addition the spin-orbit terms
+ *   linear in the spins at 2.5PN, 3PN and 3.5PN, in the variables
+ *     S_l = mu1^2 chi1 + mu2^2 chi2,   dS_l = (mu1 - mu2)(mu2 chi2 - mu1 chi1):
+ *     gamma   = (554345/1134 + 110/9 eta) S_l + (13915/84 - 10/3 eta) dS_l
+ *     phi_5  -= gamma,  phil_5 -= 3 gamma
+ *     phi_6  += pi (3760 S_l + 1490 dS_l)/3
+ *     phi_7  += (-8980424995/762048 + 6586595/756 eta - 305/36 eta^2) S_l
+ *               - (170978035/48384 - 2876425/672 eta - 4735/144 eta^2) dS_l
+ *   (terms quadratic in the spins beyond 2PN are not included).                              */
 void gwo_phase_coefficients(double eta, double mu1, double mu2, double chi1, double chi2,
                             int spin_order, double *phi, double *phil)
 {
@@ -113,6 +124,16 @@ void gwo_phase_coefficients(double eta, double mu1, double mu2, double chi1, dou
            - 6848.0 / 21.0 * log(4.0);
     phil[6] = -6848.0 / 21.0;
     phi[7] = pi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * eta * eta);
+    if (spin_order >= 2) {
+        const double sl  = mu1 * mu1 * chi1 + mu2 * mu2 * chi2;
+        const double dsl = (mu1 - mu2) * (mu2 * chi2 - mu1 * chi1);
+        const double gamma = (554345.0 / 1134.0 + 110.0 / 9.0 * eta) * sl + (13915.0 / 84.0 - 10.0 / 3.0 * eta) * dsl;
+        phi[5]  -= gamma;
+        phil[5] -= 3.0 * gamma;
+        phi[6]  += pi * (3760.0 * sl + 1490.0 * dsl) / 3.0;
+        phi[7]  += (-8980424995.0 / 762048.0 + 6586595.0 / 756.0 * eta - 305.0 / 36.0 * eta * eta) * sl
+                 - (170978035.0 / 48384.0 - 2876425.0 / 672.0 * eta - 4735.0 / 144.0 * eta * eta) * dsl;
+    }
 }
 
 /* ---- NEXT-1 option: tidal phase terms ------------------------ */
