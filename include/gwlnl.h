@@ -75,7 +75,9 @@ typedef struct gw_detector {
 } gw_detector;
 
 typedef struct gw_options {      /* NULL => { spin_order 1, isco_cut 0, max_batch 4096, phase_marginal 0, tidal_order 0 } */
-    int     spin_order;          /* 0: no spin terms; 1: 1.5PN spin-orbit + 2PN spin-spin (A7)  */
+    int     spin_order;          /* 0: no spin terms; 1: 1.5PN spin-orbit + 2PN spin-spin (A7);
+                                    2 (NEXT-1 option): also the spin-orbit terms linear
+                                    in the spins at 2.5PN, 3PN and 3.5PN                                   */
     int     isco_cut;            /* 0 (default, A6): every bin of the band is evaluated;
                                     1 (NEXT-1 option): h = 0 for f > f_ISCO =
                                     1/(6^(3/2) pi M) of the proposal's total mass                         */

@@ -249,7 +249,7 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
     if (!std::isfinite(gmst_rad)) return GW_ERR_INVALID_ARG;
     gw_options o = {1, 0, 4096, 0, 0};
     if (opt) o = *opt;
-    if (o.spin_order < 0 || o.spin_order > 1 || o.isco_cut < 0 || o.isco_cut > 1 || o.max_batch < 1 ||
+    if (o.spin_order < 0 || o.spin_order > 2 || o.isco_cut < 0 || o.isco_cut > 1 || o.max_batch < 1 ||
         o.phase_marginal < 0 || o.phase_marginal > 1 || o.tidal_order < 0 || o.tidal_order > 2)
         return GW_ERR_INVALID_ARG;
 

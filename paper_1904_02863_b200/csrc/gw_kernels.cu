@@ -199,14 +199,26 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
         const double phi2 = 3715.0 / 756.0 + 55.0 / 9.0 * eta;
         const double phi3 = -16.0 * kPi + four_beta;
         const double phi4 = 15293365.0 / 508032.0 + 27145.0 / 504.0 * eta + 3085.0 / 72.0 * eta2 + m10_sigma;
-        const double phi5 = kPi * (38645.0 / 756.0 - 65.0 / 9.0 * eta);
+        // NEXT-1 option spin_order 2: spin-orbit terms linear in the spins at 2.5PN, 3PN, 3.5PN, in the
+        // (chi_s, chi_a) coding:  S_l = (1 - 2 eta) chi_s + delta chi_a,  dS_l = -(1 - 4 eta) chi_s - delta chi_a
+        double so5 = 0.0, so6 = 0.0, so7 = 0.0;
+        if (a.spin_order >= 2) {
+            const double xs = 0.5 * (chi1 + chi2), xa = 0.5 * (chi1 - chi2);
+            const double sl  = (1.0 - 2.0 * eta) * xs + delta * xa;
+            const double dsl = -(1.0 - 4.0 * eta) * xs - delta * xa;
+            so5 = -((554345.0 / 1134.0 + 110.0 / 9.0 * eta) * sl + (13915.0 / 84.0 - 10.0 / 3.0 * eta) * dsl);
+            so6 = kPi * (3760.0 * sl + 1490.0 * dsl) / 3.0;
+            so7 = (-8980424995.0 / 762048.0 + eta * (6586595.0 / 756.0 - 305.0 / 36.0 * eta)) * sl -
+                  (170978035.0 / 48384.0 - eta * (2876425.0 / 672.0 + 4735.0 / 144.0 * eta)) * dsl;
+        }
+        const double phi5 = kPi * (38645.0 / 756.0 - 65.0 / 9.0 * eta) + so5;
         const double ph5l = 3.0 * phi5;
         constexpr double k6const = 11583231236531.0 / 4694215680.0 - 640.0 / 3.0 * kPi * kPi -
                                    6848.0 / 21.0 * (kEulerG + kLn4);
         const double phi6 = k6const + eta * (-15737765635.0 / 3048192.0 + 2255.0 / 12.0 * kPi * kPi) +
-                            76055.0 / 1728.0 * eta2 - 127825.0 / 1296.0 * eta2 * eta;
+                            76055.0 / 1728.0 * eta2 - 127825.0 / 1296.0 * eta2 * eta + so6;
         constexpr double ph6l = -6848.0 / 21.0;
-        const double phi7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * eta2);
+        const double phi7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * eta2) + so7;
         // x-form, in turns: prefactor 3/(128 eta) / (2 pi); kappa^(k-5) x^(k-5)
         const double pref = 3.0 / (128.0 * eta) / kTwoPi;
         const double kc2  = kc * kc;

@@ -343,6 +343,10 @@ def test_random_shapes(oracle, torch_cuda, seed):
     f = f0 + np.arange(M) * df
     bns = bool(rng.integers(0, 2))
     isco, marg, spin = int(rng.integers(0, 2)), int(rng.integers(0, 2)), int(rng.integers(0, 2))
+    rng3 = np.random.Generator(np.random.PCG64(999 + seed))          # one case in three each: tidal order 0, 1, 2
+    tidal = int(rng3.integers(0, 3))
+    if spin and rng3.random() < 0.5:                                 # half of the spinning cases: spin_order 2
+        spin = 2
     names = ["H1", "L1", "V1"]
     rows = []
     for i in range(n_det):
@@ -368,8 +372,6 @@ def test_random_shapes(oracle, torch_cuda, seed):
     z = rng.standard_normal((n_det, M, 2))
     d = oracle.waveform(f, dets, gmst, th[:1], spin)[0] + (z[..., 0] + 1j * z[..., 1]) * np.sqrt(S / (4 * df))
     rng2 = np.random.Generator(np.random.PCG64(777 + seed))          # every other case: a pinned launch shape
-    rng3 = np.random.Generator(np.random.PCG64(999 + seed))          # one case in three each: tidal order 0, 1, 2
-    tidal = int(rng3.integers(0, 3))
     lam = rng3.uniform(0, 5000, (B, 2))
     tkw = dict(lambdas=lam, tidal_order=tidal) if tidal else {}
     with GwContext(f, d, S, dets, gmst, spin_order=spin, max_batch=B, isco_cut=isco, phase_marginal=marg,
