@@ -61,6 +61,9 @@ constexpr double kProBins  = 14.0;
 #ifndef GW_ZERO_COPY_LNL
 #define GW_ZERO_COPY_LNL 1
 #endif
+#ifndef GW_ZERO_COPY_THETA_MAX
+#define GW_ZERO_COPY_THETA_MAX 16384   // host variant: up to this many proposals K1 reads a pinned theta buffer in place
+#endif
 #ifndef GW_SAT_WARPS
 #define GW_SAT_WARPS 2.0
 #endif
@@ -489,8 +492,17 @@ int gw_lnl_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, dou
     DeviceGuard guard(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     Workspace &w = ctx->w;
-    cudaError_t e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * ctx->t.n_param,
-                                    cudaMemcpyHostToDevice, s);
+    // A pinned theta buffer is read in place by the setup kernel (coalesced loads over the host link): one
+    // copy-engine operation and its hand-over to the kernel less per call; pageable buffers and very large batches
+    // (whose transfer the copy engine does faster) take the staged copy.
+    const double *theta_src = nullptr;
+    if (n_prop <= (int64_t)GW_ZERO_COPY_THETA_MAX) theta_src = mapped_alias(theta_host);
+    cudaError_t e = cudaSuccess;
+    if (!theta_src) {
+        e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * ctx->t.n_param,
+                            cudaMemcpyHostToDevice, s);
+        theta_src = w.theta_stage;
+    }
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     // lnL goes straight to a pinned output buffer (coalesced 8-byte stores of the finish stage over the host link):
     // one copy-engine round trip less per call; pageable buffers and `parts` take the staged copy
@@ -499,7 +511,7 @@ int gw_lnl_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, dou
 #else
     double *direct = nullptr;
 #endif
-    rc = gw_lnl_batch(ctx, n_prop, w.theta_stage, direct ? direct : w.lnl_stage, parts_out_host ? w.parts_stage : nullptr,
+    rc = gw_lnl_batch(ctx, n_prop, theta_src, direct ? direct : w.lnl_stage, parts_out_host ? w.parts_stage : nullptr,
                       cuda_stream);
     if (rc != GW_OK) return rc;
     if (!direct) e = cudaMemcpyAsync(lnl_out_host, w.lnl_stage, sizeof(double) * n_prop, cudaMemcpyDeviceToHost, s);

@@ -168,10 +168,22 @@ struct SetupArgs {
 __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
 {
     pdl_launch_dependents();          // the dependent kernel may start its table prefetch now
+    // The CTA's 32 theta rows are contiguous: stage them with coalesced loads (one pass over the rows, whether they
+    // sit in HBM or -- host variant with a pinned theta buffer -- are read over the host link), then every role
+    // reads its columns from shared memory.
+    __shared__ double s_theta[32 * GW_NPARAM_TIDAL];
+    {
+        const int64_t b_first = (int64_t)blockIdx.x * 32;
+        const int64_t rows = a.n_prop - b_first < 32 ? a.n_prop - b_first : 32;
+        const int n_load = (int)rows * a.n_param;
+        const double *src = a.theta + b_first * a.n_param;
+        for (int i = threadIdx.x; i < n_load; i += 128) s_theta[i] = src[i];
+        __syncthreads();
+    }
     const int role = threadIdx.x >> 5;
     const int64_t b = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
     if (b >= a.n_prop) return;
-    const double *th = a.theta + b * a.n_param;
+    const double *th = s_theta + (threadIdx.x & 31) * a.n_param;
     double *r = a.rec + b;
     const int64_t S = a.rec_stride;
     const double mc = th[GW_P_MC];
