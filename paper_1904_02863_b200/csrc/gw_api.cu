@@ -61,8 +61,13 @@ constexpr double kProBins  = 14.0;
 #ifndef GW_ZERO_COPY_LNL
 #define GW_ZERO_COPY_LNL 1
 #endif
+// host variant: between these batch sizes K1 reads a pinned theta buffer in place (measured: below, the small staged
+// copy is as quick and K1 is ~1 us shorter without its staging pass; above, the copy engine moves the rows faster)
+#ifndef GW_ZERO_COPY_THETA_MIN
+#define GW_ZERO_COPY_THETA_MIN 2048
+#endif
 #ifndef GW_ZERO_COPY_THETA_MAX
-#define GW_ZERO_COPY_THETA_MAX 16384   // host variant: up to this many proposals K1 reads a pinned theta buffer in place
+#define GW_ZERO_COPY_THETA_MAX 16384
 #endif
 #ifndef GW_SAT_WARPS
 #define GW_SAT_WARPS 2.0
@@ -442,8 +447,9 @@ int gw_ctx_last_kernel_ms(gw_ctx *ctx, double *setup_ms, double *main_ms)
     return GW_OK;
 }
 
-int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *lnl_out_dev,
-                 double *parts_out_dev, void *cuda_stream)
+// theta_in_host_memory: theta_dev is the device alias of a pinned host buffer (host variant, read in place)
+static int lnl_batch_impl(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, int theta_in_host_memory,
+                          double *lnl_out_dev, double *parts_out_dev, void *cuda_stream)
 {
     int rc = check_batch_args(ctx, n_prop, theta_dev, lnl_out_dev);
     if (rc != GW_OK || n_prop == 0) return rc;
@@ -456,7 +462,8 @@ int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *l
         return GW_ERR_INVALID_ARG;
     if (ctx->timing) cudaEventRecord(ctx->ev[0], s);
     cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
-                                 ctx->w.rec_stride, (double)p.lpp * ctx->t.delta_f, 1, s, &ctx->launches);
+                                 ctx->w.rec_stride, (double)p.lpp * ctx->t.delta_f, 1, theta_in_host_memory, s,
+                                 &ctx->launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     if (ctx->timing) cudaEventRecord(ctx->ev[1], s);
     e = launch_fused(ctx->t, p, n_prop, ctx->w.rec, ctx->w.rec_stride, ctx->w.partial, ctx->w.tickets, ctx->w.gpartial, ctx->w.gtickets, lnl_out_dev,
@@ -464,6 +471,12 @@ int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *l
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     if (ctx->timing) cudaEventRecord(ctx->ev[2], s);
     return GW_OK;
+}
+
+int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *lnl_out_dev,
+                 double *parts_out_dev, void *cuda_stream)
+{
+    return lnl_batch_impl(ctx, n_prop, theta_dev, 0, lnl_out_dev, parts_out_dev, cuda_stream);
 }
 
 int gw_waveform_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *h_out_dev, void *cuda_stream)
@@ -475,7 +488,7 @@ int gw_waveform_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, doub
     cudaStream_t s = (cudaStream_t)cuda_stream;
     if (ctx->timing) cudaEventRecord(ctx->ev[0], s);
     cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
-                                 ctx->w.rec_stride, ctx->t.delta_f, 0, s, &ctx->launches);
+                                 ctx->w.rec_stride, ctx->t.delta_f, 0, 0, s, &ctx->launches);
     if (e != cudaSuccess) return cuda_fail(ctx, e);
     if (ctx->timing) cudaEventRecord(ctx->ev[1], s);
     e = launch_waveform(ctx->t, n_prop, ctx->w.rec, ctx->w.rec_stride, h_out_dev, s, &ctx->launches);
@@ -496,7 +509,9 @@ int gw_lnl_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, dou
     // copy-engine operation and its hand-over to the kernel less per call; pageable buffers and very large batches
     // (whose transfer the copy engine does faster) take the staged copy.
     const double *theta_src = nullptr;
-    if (n_prop <= (int64_t)GW_ZERO_COPY_THETA_MAX) theta_src = mapped_alias(theta_host);
+    if (n_prop >= (int64_t)GW_ZERO_COPY_THETA_MIN && n_prop <= (int64_t)GW_ZERO_COPY_THETA_MAX)
+        theta_src = mapped_alias(theta_host);
+    const int in_place = theta_src != nullptr;
     cudaError_t e = cudaSuccess;
     if (!theta_src) {
         e = cudaMemcpyAsync(w.theta_stage, theta_host, sizeof(double) * n_prop * ctx->t.n_param,
@@ -511,7 +526,7 @@ int gw_lnl_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, dou
 #else
     double *direct = nullptr;
 #endif
-    rc = gw_lnl_batch(ctx, n_prop, theta_src, direct ? direct : w.lnl_stage, parts_out_host ? w.parts_stage : nullptr,
+    rc = lnl_batch_impl(ctx, n_prop, theta_src, in_place, direct ? direct : w.lnl_stage, parts_out_host ? w.parts_stage : nullptr,
                       cuda_stream);
     if (rc != GW_OK) return rc;
     if (!direct) e = cudaMemcpyAsync(lnl_out_host, w.lnl_stage, sizeof(double) * n_prop, cudaMemcpyDeviceToHost, s);

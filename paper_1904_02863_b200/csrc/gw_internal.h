@@ -104,7 +104,7 @@ cudaError_t launch_precompute(const Tables &t, const double *freqs_dev, const do
                               const double *psd_dev, double *i7_dev, cudaStream_t s, int64_t *launches);
 cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int spin_order, int64_t n_prop,
                          const double *theta_dev, double *rec, int64_t rec_stride, double rot_stride_hz,
-                         int relative_tau, cudaStream_t s, int64_t *launches);
+                         int relative_tau, int stage_theta, cudaStream_t s, int64_t *launches);
 cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, const double *rec,
                          int64_t rec_stride, double *partial, unsigned int *tickets, double *gpartial,
                          unsigned int *gtickets, double *lnl_out, double *parts_out, cudaStream_t s, int64_t *launches);

@@ -150,6 +150,7 @@ struct SetupArgs {
     double  gmst;
     int     n_det, spin_order;
     int     n_param, tidal_order;   // doubles per theta row; NEXT-1 tidal option (0 | 1 | 2)
+    int     stage_theta;            // 1: theta is pinned host memory read in place (stage rows through shared memory)
     int64_t n_prop, rec_stride;
     const double *theta;
     double *rec;
@@ -168,11 +169,11 @@ struct SetupArgs {
 __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
 {
     pdl_launch_dependents();          // the dependent kernel may start its table prefetch now
-    // The CTA's 32 theta rows are contiguous: stage them with coalesced loads (one pass over the rows, whether they
-    // sit in HBM or -- host variant with a pinned theta buffer -- are read over the host link), then every role
-    // reads its columns from shared memory.
+    // Host variant with a pinned theta buffer (stage_theta): the CTA's 32 rows are contiguous, so they are staged with
+    // coalesced loads over the host link (one pass over the rows) and every role reads its columns from shared
+    // memory.  Device-resident theta is read directly (the staging round trip would cost ~1 us per call).
     __shared__ double s_theta[32 * GW_NPARAM_TIDAL];
-    {
+    if (a.stage_theta) {
         const int64_t b_first = (int64_t)blockIdx.x * 32;
         const int64_t rows = a.n_prop - b_first < 32 ? a.n_prop - b_first : 32;
         const int n_load = (int)rows * a.n_param;
@@ -183,7 +184,7 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
     const int role = threadIdx.x >> 5;
     const int64_t b = (int64_t)blockIdx.x * 32 + (threadIdx.x & 31);
     if (b >= a.n_prop) return;
-    const double *th = s_theta + (threadIdx.x & 31) * a.n_param;
+    const double *th = a.stage_theta ? s_theta + (threadIdx.x & 31) * a.n_param : a.theta + b * a.n_param;
     double *r = a.rec + b;
     const int64_t S = a.rec_stride;
     const double mc = th[GW_P_MC];
@@ -353,9 +354,10 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
 
 cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int spin_order, int64_t n_prop,
                          const double *theta_dev, double *rec, int64_t rec_stride, double rot_stride_hz,
-                         int relative_tau, cudaStream_t s, int64_t *launches)
+                         int relative_tau, int stage_theta, cudaStream_t s, int64_t *launches)
 {
     SetupArgs a;
+    a.stage_theta = stage_theta;
     a.dets = dets; a.gmst = gmst; a.n_det = t.n_det; a.spin_order = spin_order;
     a.n_param = t.n_param; a.tidal_order = t.tidal_order;
     a.n_prop = n_prop; a.rec_stride = rec_stride; a.theta = theta_dev; a.rec = rec;

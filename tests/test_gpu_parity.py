@@ -195,12 +195,13 @@ def test_host_variants_match_device_variants(oracle, torch_cuda):
     assert np.array_equal(h_h, h_d.cpu().numpy()) and np.array_equal(lnl_only, lnl_h)
 
 
-@pytest.mark.parametrize("batch", [1, 130, 1500])
+@pytest.mark.parametrize("batch", [1, 130, 1500, 2600])
 def test_host_variant_with_pinned_output(oracle, torch_cuda, batch):
     """A pinned lnL buffer is written by the kernel itself (include/gwlnl.h, host variants): same bits as the staged
-    copy into a pageable buffer, nothing outside the n_prop entries is touched, and a sub-array offset works."""
+    copy into a pageable buffer, nothing outside the n_prop entries is touched, and a sub-array offset works.
+    From 2048 proposals a pinned theta buffer is read in place by the setup kernel (batch 2600: a ragged last CTA)."""
     torch = torch_cuda
-    cfg = inputs.CONFIGS["C1"].reduced(f_max=200.0, batch=1500)
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=200.0, batch=2600)
     f, S, dets, d, th = make_problem(oracle, cfg)
     th = th[:batch]
     with make_ctx(cfg, f, d, S, dets) as ctx:
