@@ -23,6 +23,9 @@ struct gw_ctx {
     int          last_cuda_error;
     int64_t      launches;
     int          force_lpp, force_chunks;   // gw_ctx_force_plan (0 = planner's choice)
+    int64_t      plan_n[4];        // batch sizes of the cached plans (0 = empty): a sampler calls with few distinct sizes
+    Plan         plan_of[4];       // make_plan is a pure function of n_prop for a given context and pinned shape
+    int          plan_next;
     int          timing;           // gw_ctx_kernel_timing: record events around K1 and the main kernel
     cudaEvent_t  ev[3];            // before K1, between K1 and main, after main
 };
@@ -133,6 +136,19 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
     }
     best.n_groups = best.n_chunks >= kFinishTwoLevelFrom ? (best.n_chunks + kFinishGroup - 1) / kFinishGroup : 1;
     return best;
+}
+
+// make_plan through a four-entry cache (the planner's search costs several microseconds of host time per call)
+Plan cached_plan(gw_ctx *ctx, int64_t n_prop)
+{
+    for (int i = 0; i < 4; ++i)
+        if (ctx->plan_n[i] == n_prop) return ctx->plan_of[i];
+    const Plan p = make_plan(ctx, n_prop);
+    const int slot = ctx->plan_next;
+    ctx->plan_next = (slot + 1) & 3;
+    ctx->plan_n[slot] = n_prop;
+    ctx->plan_of[slot] = p;
+    return p;
 }
 
 // upper bound of partial_need over every plan make_plan can return for n_prop <= max_batch
@@ -409,6 +425,7 @@ int gw_ctx_force_plan(gw_ctx *ctx, int lanes_per_prop, int n_chunks)
         return GW_ERR_INVALID_ARG;
     ctx->force_lpp = lanes_per_prop;
     ctx->force_chunks = n_chunks;
+    for (int i = 0; i < 4; ++i) ctx->plan_n[i] = 0;          // cached plans were made for the previous pin
     return GW_OK;
 }
 
@@ -455,7 +472,7 @@ static int lnl_batch_impl(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, 
     if (rc != GW_OK || n_prop == 0) return rc;
     DeviceGuard guard(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    const Plan p = make_plan(ctx, n_prop);
+    const Plan p = cached_plan(ctx, n_prop);
     if (partial_need(ctx, p) > ctx->w.partial_doubles || p.n_tiles > ctx->w.n_tickets) return GW_ERR_INVALID_ARG;
     if (p.n_groups > 1 && (p.n_tiles * p.n_groups * (int64_t)(2 * ctx->t.n_det) * p.props_per_cta > ctx->w.gpartial_doubles ||
                            p.n_tiles * p.n_groups > ctx->w.n_gtickets))
