@@ -149,7 +149,7 @@ int gw_lnl_batch(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, double *l
 
 /* Host-buffer variants: theta_host -> (ctx-owned device staging) -> kernels -> outputs copied back to
  * host; the stream is synchronised before returning.  Pinned host memory makes the copies asynchronous
- * with respect to the host but is not required.  When theta_host is pinned and 2048 <= n_prop <= 16384 the setup kernel reads it
+ * with respect to the host but is not required.  When theta_host is pinned and n_prop >= 2048 the setup kernel reads it
  * in place over the host link (coalesced loads, no staged copy).  When lnl_out_host is pinned (cudaHostAlloc / cudaHostRegister /
  * torch pin_memory) the kernel's finish stage stores lnL straight into it over the host link instead of a staged
  * device-to-host copy; the values are valid when the call returns either way.  The waveform variant processes the
