@@ -151,6 +151,8 @@ struct SetupArgs {
     int     n_det, spin_order;
     int     n_param, tidal_order;   // doubles per theta row; NEXT-1 tidal option (0 | 1 | 2)
     int     stage_theta;            // 1: theta is pinned host memory read in place (stage rows through shared memory)
+    int     isco_cut;               // 0: f_ISCO and the cut index are not needed
+    double  band_xi, band_x1, band_l1;   // f_min^(-1/3), f_max^(1/3), max |ln f| at the band edges (phase-domain bound)
     int64_t n_prop, rec_stride;
     const double *theta;
     double *rec;
@@ -270,8 +272,7 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
         r[(int64_t)rec_field_t12(a.n_det) * S] = t12;
         {   // domain of the integer range reduction (cis_quarter_turns: |phase| < 2^31 quarter turns): bound the
             // phase over the band by its terms at the band edges; beyond 1e9 phase units the proposal is poisoned
-            const double x0 = cbrt(a.f0), xi = 1.0 / x0, x1 = cbrt(a.f_max), tc = th[GW_P_TC];
-            const double l1 = fmax(fabs(log(a.f0)), fabs(log(a.f_max)));
+            const double xi = a.band_xi, x1 = a.band_x1, l1 = a.band_l1, tc = th[GW_P_TC];
             const double bound = fabs(r[0 * S]) * (xi * xi) * (xi * xi) * xi + fabs(r[1 * S]) * (xi * xi * xi) +
                                  fabs(r[2 * S]) * (xi * xi) + fabs(r[3 * S]) * xi + fabs(r[4 * S]) +
                                  fabs(r[5 * S]) * l1 + fabs(r[6 * S]) * x1 + fabs(r[7 * S]) * x1 * l1 +
@@ -281,6 +282,7 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
         }
         // NEXT-1 option isco_cut: f_ISCO = 1/(6^(3/2) pi M) and the last bin with f_j <= f_ISCO (-1: none).
         // The decision is taken in fp64 against the same f_j the oracle compares with.
+        if (!a.isco_cut) return;                                                    // the two fields are read by nobody
         const double f_isco = 1.0 / (6.0 * sqrt(6.0) * (kap * kap * kap));         // kappa^3 = pi M
         double jc = floor((f_isco - a.f0) / a.delta_f);
         int64_t j = jc < -1.0 ? -1 : (jc > (double)(a.n_bins - 1) ? a.n_bins - 1 : (int64_t)jc);
@@ -306,7 +308,8 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
 
     // O4: Newtonian amplitude A0 = sqrt(5/24) pi^(-2/3) (Mc Tsun)^(5/6) / (D Mpc/c)
     const double u  = mc * kTsun;
-    double a0 = sqrt(5.0 / 24.0) / cbrt(kPi * kPi) * (sqrt(u) * cbrt(u)) / (dl * kMpcSec);
+    constexpr double kAmp = 0.212787510139663399157865621657;      // sqrt(5/24) pi^(-2/3)
+    double a0 = kAmp * (sqrt(u) * cbrt(u)) / (dl * kMpcSec);
     if (!ok) a0 = __longlong_as_double(0x7ff8000000000000LL);
 
     // O6: sky frame
@@ -358,6 +361,7 @@ cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int s
 {
     SetupArgs a;
     a.stage_theta = stage_theta;
+    a.isco_cut = t.isco_cut;
     a.dets = dets; a.gmst = gmst; a.n_det = t.n_det; a.spin_order = spin_order;
     a.n_param = t.n_param; a.tidal_order = t.tidal_order;
     a.n_prop = n_prop; a.rec_stride = rec_stride; a.theta = theta_dev; a.rec = rec;
@@ -365,6 +369,8 @@ cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int s
     a.f_amp = reinterpret_cast<const double2 *>(t.planes) + 4 * t.n_pad;
     a.n_bins = t.n_bins; a.f0 = t.f0; a.delta_f = t.delta_f;
     a.f_max = t.f0 + (double)(t.n_bins - 1) * t.delta_f;
+    a.band_xi = 1.0 / cbrt(t.f0); a.band_x1 = cbrt(a.f_max);
+    a.band_l1 = fmax(fabs(log(t.f0)), fabs(log(a.f_max)));
     const unsigned blocks = (unsigned)((n_prop + 31) / 32);
     setup_kernel<<<blocks, 128, 0, s>>>(a);
     *launches += 1;
