@@ -595,17 +595,35 @@ __device__ __forceinline__ double log_bessel_i0(double x)
     return x - 0.5 * log(kTwoPi * x) + log(s);
 }
 
+// The record fields the finish stage needs (CA_I and the cut index).  The cross-chunk finish loads them before the
+// ticket round trip so that their L2 latency is not added to the last CTA's serial chain.
+template <int NDET>
+struct FinishRec { double car[NDET], cai[NDET]; int64_t jcut; };
+
 template <int NDET, bool ISCO>
-__device__ __forceinline__ void finish_proposal(const FusedArgs &a, int64_t b, const double (&zr)[NDET],
-                                                const double (&zi)[NDET])
+__device__ __forceinline__ FinishRec<NDET> load_finish_rec(const FusedArgs &a, int64_t b)
 {
-    double lnl = 0.0, sum_re = 0.0, sum_im = 0.0, sum_hh = 0.0;
-    int64_t jcut = 0;
-    if (ISCO) jcut = (int64_t)a.rec[(int64_t)rec_field_jcut(NDET) * a.rec_stride + b];
+    FinishRec<NDET> f;
+    f.jcut = 0;
+    if (ISCO) f.jcut = (int64_t)a.rec[(int64_t)rec_field_jcut(NDET) * a.rec_stride + b];
 #pragma unroll
     for (int i = 0; i < NDET; ++i) {
         const double *ri = a.rec + (int64_t)(9 + kRecPerDet * i) * a.rec_stride + b;
-        const double car = ri[a.rec_stride], cai = ri[2 * a.rec_stride];
+        f.car[i] = ri[a.rec_stride];
+        f.cai[i] = ri[2 * a.rec_stride];
+    }
+    return f;
+}
+
+template <int NDET, bool ISCO>
+__device__ __forceinline__ void finish_proposal(const FusedArgs &a, int64_t b, const FinishRec<NDET> &f,
+                                                const double (&zr)[NDET], const double (&zi)[NDET])
+{
+    double lnl = 0.0, sum_re = 0.0, sum_im = 0.0, sum_hh = 0.0;
+    const int64_t jcut = f.jcut;
+#pragma unroll
+    for (int i = 0; i < NDET; ++i) {
+        const double car = f.car[i], cai = f.cai[i];
         const double dh_re = __fma_rn(car, zr[i], cai * zi[i]);      // conj(CA) * Z
         const double dh_im = __fma_rn(car, zi[i], -(cai * zr[i]));
         const double norm  = ISCO ? (jcut >= 0 ? a.i7cum[(int64_t)i * a.n_pad + jcut] : 0.0) : a.i7[i];
@@ -885,7 +903,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
     }
 
     if (a.n_chunks == 1) {
-        if (sub == 0 && live) finish_proposal<NDET, ISCO>(a, b, zr, zi);
+        if (sub == 0 && live) finish_proposal<NDET, ISCO>(a, b, load_finish_rec<NDET, ISCO>(a, b), zr, zi);
         return;
     }
     // stage 1 -> workspace: partial[((tile*n_chunks + chunk)*2*NDET + comp)*PT + pic]
@@ -923,6 +941,9 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             }
         }
     };
+    // finish-stage record of the proposal this thread would finish (tid < PT), issued ahead of the ticket
+    const int64_t b_fin = tile * PT + (tid < PT ? tid : 0);
+    const FinishRec<NDET> frec = load_finish_rec<NDET, ISCO>(a, b_fin < a.n_prop ? b_fin : a.n_prop - 1);
     __threadfence();
     __syncthreads();
     unsigned int last_ticket = (unsigned)(a.n_chunks - 1);
@@ -979,7 +1000,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                             si[i] += sh[(c * 2 * NDET + 2 * i + 1) * PT + tid];
                         }
                     }
-                    finish_proposal<NDET, ISCO>(a, bb, sr, si);
+                    finish_proposal<NDET, ISCO>(a, bb, frec, sr, si);
                 }
             }
             if (tid == 0) a.tickets[tile] = 0u;
@@ -996,7 +1017,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                 ordered_sum(a.gpartial + (tile * a.n_groups * (int64_t)(2 * NDET)) * PT + tid, a.n_groups, sr, si);
             else
                 ordered_sum(a.partial + (tile * a.n_chunks * (int64_t)(2 * NDET)) * PT + tid, a.n_chunks, sr, si);
-            finish_proposal<NDET, ISCO>(a, bb, sr, si);
+            finish_proposal<NDET, ISCO>(a, bb, frec, sr, si);
         }
     }
     if (tid == 0) a.tickets[tile] = 0u;                      // self-reset for the next call
