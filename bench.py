@@ -35,9 +35,19 @@ METRIC = "likelihood evals/sec (fp64, waveform+lnL)"
 UNIT = "lnL/s"
 FP64_LANES_PER_SM = 64          # B200 fp64 FMA lanes per SM (37.2 TFLOP/s at 1965 MHz x 148 SMs)
 L2_FLUSH_BYTES = 256 << 20
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/*_fused_ncu_summary.md); None where no capture exists for the workload.
-NCU_DRAM_BYTES_PER_LAUNCH = {"C1": 1.82e6, "C2": 33.47e6}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel are NOT measured by this script:
+# they are carried over from the committed `ncu --set full` captures listed in profiles/dram_traffic.json (the JSON
+# line names the capture in roofline.traffic_source); null where no capture exists for the workload and options.
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "dram_traffic.json")
+
+
+def ncu_traffic(key):
+    """(bytes per launch, source) from profiles/dram_traffic.json, or (None, None)."""
+    try:
+        ent = json.load(open(TRAFFIC_FILE)).get(key)
+    except Exception:
+        ent = None
+    return (float(ent["bytes_per_launch"]), ent["source"]) if ent else (None, None)
 
 
 def parse_workload(spec):
@@ -46,6 +56,13 @@ def parse_workload(spec):
     cfg = inputs.CONFIGS[name]
     batch = int(b) if b else (4096 if name == "C4" else cfg.batch)
     return name, cfg, batch
+
+
+def executed_per_bin(n_det, tidal_order=0):
+    """fp64 instructions the fused kernel EXECUTES per (proposal, bin): 9 phase + 12 sincos +
+    4 for the reference detector + 8 per further detector (+4 with the tidal option) -- 41 at N_det = 3.  The closed
+    form <h|h> and the trimmed sincos are algorithmic savings, so this is below W_alg."""
+    return 9 + 12 + 4 + 8 * (n_det - 1) + (4 if tidal_order else 0)
 
 
 def walg_per_bin(n_det, tidal_order=0):
@@ -197,9 +214,10 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if local == 0 and os.path.exists(csrc_build.NVCC):
         csrc_build.build()             # no-op when csrc/libgwlnl.so is newer than its sources
+        csrc_build.build_probe()
     if world > 1:
         dist.barrier()                 # nobody loads the library while local rank 0 may be rebuilding it
-    from paper_1904_02863_b200 import GwContext, binding
+    from paper_1904_02863_b200 import GwContext, binding, probes
     n_gpus = world
 
     name, cfg, batch = parse_workload(args.workload)
@@ -227,8 +245,8 @@ def run_ours(args):
     plan = ctx.plan(B)
 
     # ---- clock ramp + measured fp64 FMA rate (the measured roofline denominator) ----
-    fma_rate, _ = binding.probe_fp64_fma_rate(1 << 14)
-    fma_rate, _ = binding.probe_fp64_fma_rate(1 << 15)
+    fma_rate, _ = probes.fp64_fma_rate(1 << 14)
+    fma_rate, _ = probes.fp64_fma_rate(1 << 15)
 
     def step():
         ctx.lnl_batch(thd, out=lnl)
@@ -274,6 +292,7 @@ def run_ours(args):
     ctx.kernel_timing(False)
     fused_ms = float(np.mean(k_ms))
     walg = walg_per_bin(n_det, args.tidal_order)
+    wexe = executed_per_bin(n_det, args.tidal_order)
     pairs = float(B) * M                                   # (proposal, bin) pairs with algorithmic work
     if args.isco_cut:                                      # only bins up to each proposal's f_ISCO carry work
         from paper_1904_02863_b200.inputs import P_MC, P_Q
@@ -290,8 +309,14 @@ def run_ours(args):
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     peak = n_sm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    plain = not (args.isco_cut or args.phase_marginal or args.tidal_order)
+    traffic, traffic_source = ncu_traffic(name) if (B == cfg.batch and plain and world == 1) else (None, None)
     roofline = {"bound": "alu", "kernel": "fused_kernel<%d>" % n_det, "achieved": achieved, "peak": peak,
-                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(name) if B == cfg.batch else None,
+                "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source,
+                "frac_note": "frac credits the declared algorithmic work W_alg (SURVEY.md 8(d)); frac_executed counts the "
+                             "fp64 instructions the kernel issues and is the fraction of raw fp64-pipe issue slots",
+                "executed_fp64_per_prop_bin": wexe, "frac_executed": achieved / peak * wexe / walg,
+                "kernel_ms_median": float(np.median(k_ms)), "kernel_ms_best": float(np.min(k_ms)),
                 "peak_source": "derived: %d SMs x %d fp64 FMA lanes x 2 flop x %.0f MHz (%s)"
                                % (n_sm, FP64_LANES_PER_SM, sm_max,
                                   "MEASURED_PEAKS.json sm_max_mhz" if "sm_max_mhz" in peaks else "fallback clock, B200_PROFILING.md"),
@@ -359,11 +384,15 @@ def run_ours(args):
         ctx.kernel_timing(False)
         gbs = wb * n_det * M * 16 / (np.mean(w_ms) * 1e-3) / 1e9
         hbm = float(peaks.get("hbm_gbs", 6650.0))
-        extra["waveform_kernel"] = {"proposals": wb, "bytes_stored": wb * n_det * M * 16, "kernel_ms": float(np.mean(w_ms)),
-                                    "achieved_GBps": gbs, "hbm_peak_GBps": hbm,
-                                    "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)",
-                                    "frac": gbs / hbm}
         del h
+        store_gbs, _ = probes.store_bandwidth(2 << 30, 10)          # the pure-store ceiling, same run
+        extra["waveform_kernel"] = {"proposals": wb, "bytes_stored": wb * n_det * M * 16, "kernel_ms": float(np.mean(w_ms)),
+                                    "kernel_ms_median": float(np.median(w_ms)), "kernel_ms_best": float(np.min(w_ms)),
+                                    "achieved_GBps": gbs, "hbm_peak_GBps": hbm,
+                                    "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy: read + write)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)",
+                                    "frac": gbs / hbm,
+                                    "pure_store_ceiling_GBps": store_gbs, "frac_of_pure_store": gbs / store_gbs,
+                                    "pure_store_source": "gw_probe_store_bandwidth: 2 GiB of 16-byte streaming stores, best of 10, this run"}
 
     # ---- CPU baseline: the oracle as it stands on this box's host cores (rank 0, N = 1 only) ----
     cpu = None
@@ -380,7 +409,9 @@ def run_ours(args):
     ctx.close()
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n_gpus, "steps": args.steps,
-                "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+                "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps,
+                "ms_per_step_median": float(np.median(step_ms)), "ms_per_step_best": float(np.min(step_ms)),
+                "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": f"{name}: {n_det} det x {M} bins x {B} proposals per GPU",
                            "global_batch": B * world, "bins": M, "detectors": n_det, "parallelism": f"proposals sharded x{world}",

@@ -49,7 +49,7 @@
 extern "C" {
 #endif
 
-#define GW_ABI_VERSION 3
+#define GW_ABI_VERSION 4
 
 enum {
     GW_OK              =  0,
@@ -169,36 +169,16 @@ int gw_ctx_info(const gw_ctx *ctx, int64_t *n_bins, int *n_det, double *delta_f,
 int gw_ctx_n_param(const gw_ctx *ctx);
 
 /* The launch shape gw_lnl_batch would use for n_prop proposals (what bench.py reports and what fixes
- * the summation order): lanes per proposal, proposals per CTA, number of frequency chunks, CTAs.       */
+ * the summation order): lanes per proposal, proposals per CTA, number of frequency chunks, CTAs.  The aids that pin
+ * this shape or time the kernels individually are declared in gwlnl_tuning.h, outside this boundary.          */
 int gw_ctx_plan(const gw_ctx *ctx, int64_t n_prop, int *lanes_per_prop, int *props_per_cta,
                 int *n_chunks, int64_t *n_ctas);
-
-/* Testing / tuning aid: pin the launch shape gw_lnl_batch uses (lanes_per_prop in {1,2,4,8,16,32}, n_chunks >= 1
- * frequency chunks per proposal tile); 0 leaves that choice to the planner.  A pinned shape whose partial sums do not
- * fit the reserved workspace makes gw_lnl_batch return GW_ERR_INVALID_ARG.                              */
-int gw_ctx_force_plan(gw_ctx *ctx, int lanes_per_prop, int n_chunks);
 
 /* I7[n_det], the per-detector norm the precompute kernel produced (for tests of kernel K0).            */
 int gw_ctx_norms(const gw_ctx *ctx, double *i7_host);
 
 /* Number of kernel launches the library has enqueued through this context so far.                      */
 int64_t gw_ctx_launch_count(const gw_ctx *ctx);
-
-/* Measurement aid: when enabled, the *_batch calls record CUDA events on their stream before the setup
- * kernel, between the setup kernel and the main (fused or waveform) kernel, and after it.  The event between
- * the two launches removes their programmatic overlap, so enable it only for kernel-level timing.
- * gw_ctx_last_kernel_ms waits for the most recent call and returns the two durations.                  */
-int gw_ctx_kernel_timing(gw_ctx *ctx, int enable);
-int gw_ctx_last_kernel_ms(gw_ctx *ctx, double *setup_ms, double *main_ms);
-
-/* Register-resident fp64 rate microbenchmark on the current device (8 independent chains per thread, 64 warps
- * per SM): enqueues `n_iter` rounds of 64 instructions per thread and reports achieved fp64 FMA/s -- the measured
- * roofline denominator (MEASURED_PEAKS.json has no fp64 entry).  `mode` selects the operand pattern:
- * 0 = fma(v, imm, imm) (pipe peak); 1 = fma(a, b, v) with three distinct register operands; 2 = three register
- * operands of which one is shared by consecutive instructions; 3 = mma.sync m8n8k4 f64; 4, 5 = mode 0 with 8 or 16
- * independent integer instructions beside every 8 DFMA (does the fp64 rate drop?).  Synchronises.
- * Errors: GW_ERR_INVALID_ARG, GW_ERR_CUDA, GW_ERR_ARCH.                                                 */
-int gw_probe_fp64_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, void *cuda_stream);
 
 const char *gw_strerror(int code);
 int gw_last_cuda_error(const gw_ctx *ctx);      /* a cudaError_t value, 0 if none                         */

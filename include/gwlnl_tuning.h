@@ -1,0 +1,31 @@
+/*
+ * gwlnl_tuning.h -- testing / tuning / measurement aids exported by csrc/libgwlnl.so next to the product boundary
+ * of gwlnl.h.  They are not part of the surface SURVEY.md 8(b) lists: the tests use them to force every launch shape
+ * of the fused kernel, bench.py to time the kernels one by one.  Same conventions as gwlnl.h (int return codes,
+ * opaque context, no allocation in the batch path).
+ */
+#ifndef GWLNL_TUNING_H
+#define GWLNL_TUNING_H
+
+#include "gwlnl.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Testing / tuning aid: pin the launch shape gw_lnl_batch uses (lanes_per_prop in {1,2,4,8,16,32}, n_chunks >= 1
+ * frequency chunks per proposal tile); 0 leaves that choice to the planner.  A pinned shape whose partial sums do not
+ * fit the reserved workspace makes gw_lnl_batch return GW_ERR_INVALID_ARG.                              */
+int gw_ctx_force_plan(gw_ctx *ctx, int lanes_per_prop, int n_chunks);
+
+/* Measurement aid: when enabled, the *_batch calls record CUDA events on their stream before the setup
+ * kernel, between the setup kernel and the main (fused or waveform) kernel, and after it.  The event between
+ * the two launches removes their programmatic overlap, so enable it only for kernel-level timing.
+ * gw_ctx_last_kernel_ms waits for the most recent call and returns the two durations.                  */
+int gw_ctx_kernel_timing(gw_ctx *ctx, int enable);
+int gw_ctx_last_kernel_ms(gw_ctx *ctx, double *setup_ms, double *main_ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GWLNL_TUNING_H */

@@ -24,8 +24,10 @@ GW_OK, GW_ERR_INVALID_ARG, GW_ERR_ALLOC, GW_ERR_CUDA, GW_ERR_ARCH = 0, -1, -2, -
 EXPORTS = (
     "gw_ctx_create", "gw_ctx_reserve", "gw_waveform_batch", "gw_lnl_batch", "gw_lnl_batch_host",
     "gw_waveform_batch_host", "gw_ctx_destroy", "gw_ctx_info", "gw_ctx_n_param", "gw_ctx_plan", "gw_ctx_norms",
-    "gw_ctx_launch_count", "gw_ctx_force_plan", "gw_ctx_kernel_timing", "gw_ctx_last_kernel_ms", "gw_probe_fp64_fma_rate", "gw_strerror", "gw_last_cuda_error", "gw_abi_version",
+    "gw_ctx_launch_count", "gw_strerror", "gw_last_cuda_error", "gw_abi_version",
 )
+# include/gwlnl_tuning.h: testing / tuning aids exported by the same library, outside the product boundary
+TUNING_EXPORTS = ("gw_ctx_force_plan", "gw_ctx_kernel_timing", "gw_ctx_last_kernel_ms")
 
 
 class GwError(RuntimeError):
@@ -46,8 +48,8 @@ class gw_options(ctypes.Structure):
 
 
 def lib_path() -> str:
-    """csrc/libgwlnl.so, or the file named by $GWLNL_LIBRARY (a differently tuned build of the same sources)."""
-    return os.environ.get("GWLNL_LIBRARY") or os.path.join(_HERE, "csrc", "libgwlnl.so")
+    """csrc/libgwlnl.so, built in-tree by csrc/build.py (no environment-variable dispatch)."""
+    return os.path.join(_HERE, "csrc", "libgwlnl.so")
 
 
 _lib = None
@@ -82,12 +84,11 @@ def load_library():
     lib.gw_ctx_force_plan.argtypes = [vp, ci, ci]
     lib.gw_ctx_kernel_timing.argtypes = [vp, ci]
     lib.gw_ctx_last_kernel_ms.argtypes = [vp, P(dbl), P(dbl)]
-    lib.gw_probe_fp64_fma_rate.argtypes = [ci, ci, P(dbl), P(dbl), vp]
     lib.gw_strerror.argtypes = [ci]
     lib.gw_strerror.restype = ctypes.c_char_p
     lib.gw_last_cuda_error.argtypes = [vp]
     lib.gw_abi_version.argtypes = []
-    for name in EXPORTS:
+    for name in EXPORTS + TUNING_EXPORTS:
         if name not in ("gw_strerror", "gw_ctx_launch_count"):
             getattr(lib, name).restype = ci
     _lib = lib
@@ -240,6 +241,27 @@ class GwContext:
                           f"want a contiguous CUDA float64 tensor [n_prop][{self.n_param}]")
         return theta
 
+    @staticmethod
+    def _out_dev(t, n_elem, like, what, dtype=None):
+        """A caller-supplied output tensor must be CUDA, contiguous, of the right dtype and at least n_elem long,
+        on theta's device: the kernels store through its raw pointer."""
+        import torch
+        dtype = dtype or torch.float64
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()
+                and t.numel() >= n_elem and t.device == like.device):
+            raise GwError(GW_ERR_INVALID_ARG, what,
+                          f"want a contiguous CUDA {dtype} tensor of at least {n_elem} elements on {like.device}")
+        return t
+
+    @staticmethod
+    def _out_host(a, n_elem, what, dtype=np.float64):
+        """A caller-supplied host output must be a C-contiguous, writeable numpy array of the right dtype and size."""
+        if not (isinstance(a, np.ndarray) and a.dtype == dtype and a.flags["C_CONTIGUOUS"] and a.flags["WRITEABLE"]
+                and a.size >= n_elem):
+            raise GwError(GW_ERR_INVALID_ARG, what,
+                          f"want a C-contiguous writeable numpy {np.dtype(dtype).name} array of at least {n_elem} elements")
+        return a
+
     def lnl_batch(self, theta, out=None, parts=None, want_parts: bool = False, stream=None):
         """gw_lnl_batch: theta [B][11] CUDA f64 -> lnL [B] (and parts [B][n_det][3]).  Asynchronous."""
         import torch
@@ -247,8 +269,12 @@ class GwContext:
         n = th.shape[0]
         if out is None:
             out = torch.empty(n, dtype=torch.float64, device=th.device)
+        else:
+            self._out_dev(out, n, th, "lnl_batch out")
         if parts is None and want_parts:
             parts = torch.empty((n, self.n_det, 3), dtype=torch.float64, device=th.device)
+        elif parts is not None:
+            self._out_dev(parts, n * self.n_det * 3, th, "lnl_batch parts")
         rc = self._lib.gw_lnl_batch(self._h, n, th.data_ptr(), out.data_ptr(),
                                     parts.data_ptr() if parts is not None else None, _stream_ptr(stream))
         _check(rc, "gw_lnl_batch", self._h)
@@ -261,6 +287,8 @@ class GwContext:
         n = th.shape[0]
         if out is None:
             out = torch.empty((n, self.n_det, self.n_bins), dtype=torch.complex128, device=th.device)
+        else:
+            self._out_dev(out, n * self.n_det * self.n_bins, th, "waveform_batch out", torch.complex128)
         rc = self._lib.gw_waveform_batch(self._h, n, th.data_ptr(), out.data_ptr(), _stream_ptr(stream))
         _check(rc, "gw_waveform_batch", self._h)
         return out
@@ -272,8 +300,12 @@ class GwContext:
         n = th.shape[0]
         if out is None:
             out = np.empty(n)
+        else:
+            self._out_host(out, n, "lnl_batch_host out")
         if parts is None and want_parts:
             parts = np.empty((n, self.n_det, 3))
+        elif parts is not None:
+            self._out_host(parts, n * self.n_det * 3, "lnl_batch_host parts")
         rc = self._lib.gw_lnl_batch_host(self._h, n, _host_ptr(th), _host_ptr(out),
                                          _host_ptr(parts) if parts is not None else None, _stream_ptr(stream))
         _check(rc, "gw_lnl_batch_host", self._h)
@@ -284,18 +316,11 @@ class GwContext:
         n = th.shape[0]
         if out is None:
             out = np.empty((n, self.n_det, self.n_bins), dtype=np.complex128)
+        else:
+            self._out_host(out, n * self.n_det * self.n_bins, "waveform_batch_host out", np.complex128)
         rc = self._lib.gw_waveform_batch_host(self._h, n, _host_ptr(th), _host_ptr(out), _stream_ptr(stream))
         _check(rc, "gw_waveform_batch_host", self._h)
         return out
-
-
-def probe_fp64_fma_rate(n_iter: int = 4096, mode: int = 0, stream=None):
-    """(fp64 FMA/s, elapsed ms) of the register-resident probe kernel; mode: see gw_probe_fp64_fma_rate."""
-    lib = load_library()
-    rate, ms = ctypes.c_double(), ctypes.c_double()
-    _check(lib.gw_probe_fp64_fma_rate(int(n_iter), int(mode), ctypes.byref(rate), ctypes.byref(ms), _stream_ptr(stream)),
-           "gw_probe_fp64_fma_rate")
-    return rate.value, ms.value
 
 
 def waveform_for_inputs(freqs, det_rows, gmst, theta, spin_order):

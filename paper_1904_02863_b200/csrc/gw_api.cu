@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "gw_internal.h"
+#include "../../include/gwlnl_tuning.h"
 
 using namespace gw;
 
@@ -216,6 +217,9 @@ int reserve_impl(gw_ctx *ctx, int64_t max_batch)
     ctx->w = w;
     ctx->w.h_stage = old_h;
     ctx->w.h_stage_doubles = old_h_doubles;
+    // The two memsets above ran on the legacy default stream, which is not ordered against non-blocking streams:
+    // the zeroed ticket counters must be in place before any batch call on any stream can read them.
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return cuda_fail(ctx, e);
     return GW_OK;
 }
 
@@ -588,16 +592,6 @@ int gw_waveform_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host
     }
     if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(ctx, e);
     return GW_OK;
-}
-
-int gw_probe_fp64_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, void *cuda_stream)
-{
-    if (n_iter < 1 || mode < 0 || mode > 5) return GW_ERR_INVALID_ARG;
-    int dev = 0;
-    cudaDeviceProp prop;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return GW_ERR_CUDA;
-    if (prop.major != 10) return GW_ERR_ARCH;
-    return probe_fma_rate(n_iter, mode, fma_per_s, elapsed_ms, (cudaStream_t)cuda_stream) == cudaSuccess ? GW_OK : GW_ERR_CUDA;
 }
 
 } // extern "C"

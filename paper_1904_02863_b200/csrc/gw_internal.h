@@ -32,6 +32,11 @@ constexpr int kMinCtas    = GW_MIN_CTAS;    // __launch_bounds__ residency targe
 constexpr int kStageBins  = GW_STAGE_BINS;  // bins per shared-memory stage of the fused kernel
 constexpr int kStages     = GW_STAGES;      // stage ring depth
 constexpr int kUnroll     = GW_UNROLL;      // bins per unrolled trip of the fused hot loop
+// The lanes-interleaved sweep keeps each lane's bins at stride lpp <= 32 across stage boundaries, and every stage
+// plane is one bulk copy of 16-byte elements.
+static_assert(kStageBins % 32 == 0, "GW_STAGE_BINS must be a multiple of 32 (lanes-interleaved sweep, f_last seed)");
+static_assert((kStageBins * 16) % 128 == 0, "stage planes must keep the 128-byte alignment of the bulk copies");
+static_assert(kStages >= 2 && kThreads % 32 == 0 && kThreads <= 1024, "stage ring / CTA shape");
 constexpr int kBasis      = 8;     // per-bin phase basis values (4 planes of 2)
 constexpr int kBasisPlanes = 5;    // (x^-5,x^-3) (x^-2,x^-1) (ln f,x) (x ln f,x^2) (f,f^-7/6)
 constexpr int kFinishGroup = 16;   // chunks per group of the two-level finish
@@ -113,6 +118,5 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
 cudaError_t configure_kernels(int *fused_ctas_per_sm);      // smem attributes + occupancy query (per n_det below)
 int         fused_ctas_per_sm(int n_det);
 size_t      fused_smem_bytes(int n_det);
-cudaError_t probe_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, cudaStream_t s);
 
 } // namespace gw

@@ -153,6 +153,7 @@ struct SetupArgs {
     int     stage_theta;            // 1: theta is pinned host memory read in place (stage rows through shared memory)
     int     isco_cut;               // 0: f_ISCO and the cut index are not needed
     double  band_xi, band_x1, band_l1;   // f_min^(-1/3), f_max^(1/3), max |ln f| at the band edges (phase-domain bound)
+    double  max_dt;                      // max_I |dt_I| over the detectors [s]: the phase carries f (t_c + dt_I)
     int64_t n_prop, rec_stride;
     const double *theta;
     double *rec;
@@ -276,7 +277,7 @@ __global__ void __launch_bounds__(128) setup_kernel(const SetupArgs a)
             const double bound = fabs(r[0 * S]) * (xi * xi) * (xi * xi) * xi + fabs(r[1 * S]) * (xi * xi * xi) +
                                  fabs(r[2 * S]) * (xi * xi) + fabs(r[3 * S]) * xi + fabs(r[4 * S]) +
                                  fabs(r[5 * S]) * l1 + fabs(r[6 * S]) * x1 + fabs(r[7 * S]) * x1 * l1 +
-                                 fabs(r[8 * S]) * x1 * x1 + kPhaseScale * (fabs(tc) + 1.0) * a.f_max +
+                                 fabs(r[8 * S]) * x1 * x1 + kPhaseScale * (fabs(tc) + a.max_dt + 1.0) * a.f_max +
                                  (fabs(t10) + fabs(t12) * x1 * x1) * (x1 * x1) * (x1 * x1) * x1;
             if (!(bound < 1.0e9) || !tidal_ok) r[4 * S] = __longlong_as_double(0x7ff8000000000000LL);
         }
@@ -371,6 +372,13 @@ cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int s
     a.f_max = t.f0 + (double)(t.n_bins - 1) * t.delta_f;
     a.band_xi = 1.0 / cbrt(t.f0); a.band_x1 = cbrt(a.f_max);
     a.band_l1 = fmax(fabs(log(t.f0)), fabs(log(a.f_max)));
+    a.max_dt = 0.0;                      // FIXED: the given delay; GEOMETRIC: |dt| <= |r| / c
+    for (int i = 0; i < t.n_det; ++i) {
+        const DetGeom &g = dets.d[i];
+        const double m = g.kind == GW_DET_FIXED ? fabs(g.dt_s)
+                                                : sqrt(g.rc[0] * g.rc[0] + g.rc[1] * g.rc[1] + g.rc[2] * g.rc[2]);
+        a.max_dt = fmax(a.max_dt, m);
+    }
     const unsigned blocks = (unsigned)((n_prop + 31) / 32);
     setup_kernel<<<blocks, 128, 0, s>>>(a);
     *launches += 1;
@@ -1121,99 +1129,5 @@ cudaError_t configure_kernels(int *out)
     return cudaSuccess;
 }
 int fused_ctas_per_sm(int n_det) { return (n_det >= 1 && n_det <= GW_MAX_DET) ? g_ctas_per_sm[n_det] : 0; }
-
-// =====================================================================================================
-// fp64 rate probe: 8 independent register-resident chains per thread, 64 warps per SM.
-//   mode 0: v = fma(v, imm, imm)          one register operand            -> the pipe's peak
-//   mode 1: v = fma(a_i, b_i, v)          three distinct register operands (what a dot product needs)
-//   mode 2: v = fma(a_i, m, v)            three register operands, one shared by consecutive instructions
-//   mode 3: mma.sync m8n8k4 f64 (DMMA)    256 FMA per warp instruction
-// Measured on B200 (profiles/r1_fp64_operand_probe.md): modes 0/2/3 reach ~18.5e12 FMA/s, mode 1 only 2/3 of
-// it: a DFMA that reads three distinct 64-bit registers occupies the pipe for 3 cycles instead of 2, and DMMA
-// shares the same pipe.  This is the roofline the fused kernel is read against.
-// =====================================================================================================
-template <int MODE>
-__global__ void __launch_bounds__(256) fma_probe_kernel(int n_iter, const double *in, double *sink)
-{
-    double v[8], a[8], b[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        v[i] = in[threadIdx.x + i]; a[i] = in[64 + threadIdx.x + 3 * i]; b[i] = in[128 + threadIdx.x + 5 * i];
-    }
-    const double m = in[7];
-    unsigned int x[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) x[i] = threadIdx.x * 2654435761u + i;
-    for (int it = 0; it < n_iter; ++it) {
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            // modes 4, 5: independent integer instructions (one IMAD + one LOP3 per element) beside the 8 DFMA:
-            // are their issue slots free?
-            if (MODE == 4 || MODE == 5) {
-#pragma unroll
-                for (int i = 0; i < (MODE == 4 ? 4 : 8); ++i) x[i] = (x[i] ^ (unsigned)it) * 3u + 0x9e3779b9u;
-            }
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                if (MODE == 0 || MODE == 4 || MODE == 5) v[i] = __fma_rn(v[i], 0.999999, 1e-9);
-                if (MODE == 1) v[i] = __fma_rn(a[i], b[i], v[i]);
-                if (MODE == 2) v[i] = __fma_rn(a[i], m, v[i]);
-                if (MODE == 3)
-                    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                                 : "+d"(v[i]), "+d"(b[i]) : "d"(a[0]), "d"(m));
-            }
-        }
-    }
-    double r = 0.0;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) r += v[i] + b[i];
-    if (MODE == 4 || MODE == 5) {
-        unsigned int y = 0;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) y ^= x[i];
-        if (y == 0x12345u) r = 123.456;
-    }
-    if (r == 123.456) sink[0] = r;                           // never true; keeps the chains alive
-}
-
-cudaError_t probe_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, cudaStream_t s)
-{
-    int dev = 0, sms = 0;
-    cudaError_t e;
-    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    double *buf = nullptr;
-    if ((e = cudaMalloc(&buf, 1024 * sizeof(double))) != cudaSuccess) return e;
-    cudaMemsetAsync(buf, 0, 1024 * sizeof(double), s);
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    const int blocks = sms * 8;
-    auto launch = [&](int n) {
-        switch (mode) {
-        case 1:  fma_probe_kernel<1><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
-        case 2:  fma_probe_kernel<2><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
-        case 3:  fma_probe_kernel<3><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
-        case 4:  fma_probe_kernel<4><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
-        case 5:  fma_probe_kernel<5><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
-        default: fma_probe_kernel<0><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
-        }
-    };
-    launch(n_iter / 8 + 1);                                  // warm-up
-    cudaEventRecord(e0, s);
-    launch(n_iter);
-    cudaEventRecord(e1, s);
-    e = cudaEventSynchronize(e1);
-    float ms = 0.f;
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(buf);
-    if (e != cudaSuccess) return e;
-    // per thread and iteration: 64 instructions; a DMMA instruction is 256 FMA per warp = 8 per lane
-    const double per_instr = (mode == 3) ? 8.0 : 1.0;
-    const double fmas = (double)blocks * 256.0 * (double)n_iter * 64.0 * per_instr;
-    if (fma_per_s) *fma_per_s = fmas / (ms * 1e-3);
-    if (elapsed_ms) *elapsed_ms = ms;
-    return cudaGetLastError();
-}
 
 } // namespace gw

@@ -1,0 +1,199 @@
+// gw_probe.cu -- measurement aids, built into their own library (csrc/libgwprobe.so; include/gwprobe.h).  NOT part of
+// the product library libgwlnl.so: bench.py uses them for the measured roofline denominators that
+// MEASURED_PEAKS.json lacks (fp64 FMA rate; pure-store and pure-load HBM bandwidth), and
+// `python -m paper_1904_02863_b200.probes` prints them.  sm_100a only.  Shares nothing with oracle/.
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/gwprobe.h"
+
+namespace {
+
+// =====================================================================================================
+// fp64 rate probe: 8 independent register-resident chains per thread, 64 warps per SM.
+//   mode 0: v = fma(v, imm, imm)          one register operand            -> the pipe's peak
+//   mode 1: v = fma(a_i, b_i, v)          three distinct register operands (what a dot product needs)
+//   mode 2: v = fma(a_i, m, v)            three register operands, one shared by consecutive instructions
+//   mode 3: mma.sync m8n8k4 f64 (DMMA)    256 FMA per warp instruction
+// Measured on B200 (profiles/r1_fp64_operand_probe.md): modes 0/2/3 reach ~18.5e12 FMA/s, mode 1 only 2/3 of
+// it: a DFMA that reads three distinct 64-bit registers occupies the pipe for 3 cycles instead of 2, and DMMA
+// shares the same pipe.  This is the roofline the fused kernel is read against.
+// =====================================================================================================
+template <int MODE>
+__global__ void __launch_bounds__(256) fma_probe_kernel(int n_iter, const double *in, double *sink)
+{
+    double v[8], a[8], b[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        v[i] = in[threadIdx.x + i]; a[i] = in[64 + threadIdx.x + 3 * i]; b[i] = in[128 + threadIdx.x + 5 * i];
+    }
+    const double m = in[7];
+    unsigned int x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = threadIdx.x * 2654435761u + i;
+    for (int it = 0; it < n_iter; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            // modes 4, 5: independent integer instructions (one IMAD + one LOP3 per element) beside the 8 DFMA:
+            // are their issue slots free?
+            if (MODE == 4 || MODE == 5) {
+#pragma unroll
+                for (int i = 0; i < (MODE == 4 ? 4 : 8); ++i) x[i] = (x[i] ^ (unsigned)it) * 3u + 0x9e3779b9u;
+            }
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if (MODE == 0 || MODE == 4 || MODE == 5) v[i] = __fma_rn(v[i], 0.999999, 1e-9);
+                if (MODE == 1) v[i] = __fma_rn(a[i], b[i], v[i]);
+                if (MODE == 2) v[i] = __fma_rn(a[i], m, v[i]);
+                if (MODE == 3)
+                    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                 : "+d"(v[i]), "+d"(b[i]) : "d"(a[0]), "d"(m));
+            }
+        }
+    }
+    double r = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) r += v[i] + b[i];
+    if (MODE == 4 || MODE == 5) {
+        unsigned int y = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) y ^= x[i];
+        if (y == 0x12345u) r = 123.456;
+    }
+    if (r == 123.456) sink[0] = r;                           // never true; keeps the chains alive
+}
+
+static cudaError_t probe_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, cudaStream_t s)
+{
+    int dev = 0, sms = 0;
+    cudaError_t e;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    double *buf = nullptr;
+    if ((e = cudaMalloc(&buf, 1024 * sizeof(double))) != cudaSuccess) return e;
+    cudaMemsetAsync(buf, 0, 1024 * sizeof(double), s);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = sms * 8;
+    auto launch = [&](int n) {
+        switch (mode) {
+        case 1:  fma_probe_kernel<1><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        case 2:  fma_probe_kernel<2><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        case 3:  fma_probe_kernel<3><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        case 4:  fma_probe_kernel<4><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        case 5:  fma_probe_kernel<5><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        default: fma_probe_kernel<0><<<blocks, 256, 0, s>>>(n, buf, buf + 512); break;
+        }
+    };
+    launch(n_iter / 8 + 1);                                  // warm-up
+    cudaEventRecord(e0, s);
+    launch(n_iter);
+    cudaEventRecord(e1, s);
+    e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (e != cudaSuccess) return e;
+    // per thread and iteration: 64 instructions; a DMMA instruction is 256 FMA per warp = 8 per lane
+    const double per_instr = (mode == 3) ? 8.0 : 1.0;
+    const double fmas = (double)blocks * 256.0 * (double)n_iter * 64.0 * per_instr;
+    if (fma_per_s) *fma_per_s = fmas / (ms * 1e-3);
+    if (elapsed_ms) *elapsed_ms = ms;
+    return cudaGetLastError();
+}
+
+
+// =====================================================================================================
+// HBM bandwidth probes: a pure-store stream (what the waveform kernel does: 16-byte streaming stores, no reads) and
+// a pure-load stream (what the population kernel does: 16-byte loads, a reduction, no stores).  One element per
+// thread and trip, grid-stride, the buffer far larger than the 126 MB L2.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) store_probe_kernel(double2 *__restrict__ dst, int64_t n16, double v)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride)
+        __stcs(dst + i, make_double2(v, (double)i));
+}
+
+__global__ void __launch_bounds__(256) load_probe_kernel(const double2 *__restrict__ src, int64_t n16, double *sink)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    double acc = 0.0;
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 3 * stride < n16; i += 4 * stride) {          // four independent 16-byte loads in flight per thread
+        const double2 a = __ldcs(src + i), b = __ldcs(src + i + stride), c = __ldcs(src + i + 2 * stride),
+                      d = __ldcs(src + i + 3 * stride);
+        acc += (a.x + b.x) + (c.x + d.x) + (a.y + b.y) + (c.y + d.y);
+    }
+    for (; i < n16; i += stride) { const double2 a = __ldcs(src + i); acc += a.x + a.y; }
+    if (acc == 123.456) sink[0] = acc;                       // never true for the zero-filled buffer; keeps the loads
+}
+
+cudaError_t probe_bandwidth(int store, int64_t bytes, int n_rep, double *gb_per_s, double *best_ms, cudaStream_t s)
+{
+    int dev = 0, sms = 0;
+    cudaError_t e;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    double2 *buf = nullptr;
+    double *sink = nullptr;
+    const int64_t n16 = bytes / 16;
+    if ((e = cudaMalloc(&buf, (size_t)n16 * 16)) != cudaSuccess) return e;
+    if ((e = cudaMalloc(&sink, 64)) != cudaSuccess) { cudaFree(buf); return e; }
+    cudaMemsetAsync(buf, 0, (size_t)n16 * 16, s);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = sms * 8;                              // 8 resident 256-thread CTAs per SM
+    float best = 1e30f;
+    for (int r = 0; r < n_rep + 1 && e == cudaSuccess; ++r) {   // first pass is the warm-up
+        cudaEventRecord(e0, s);
+        if (store) store_probe_kernel<<<blocks, 256, 0, s>>>(buf, n16, (double)r);
+        else       load_probe_kernel<<<blocks, 256, 0, s>>>(buf, n16, sink);
+        cudaEventRecord(e1, s);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(buf); cudaFree(sink);
+    if (e != cudaSuccess) return e;
+    if (gb_per_s) *gb_per_s = (double)n16 * 16.0 / (best * 1e-3) / 1e9;
+    if (best_ms) *best_ms = best;
+    return cudaGetLastError();
+}
+
+bool arch_ok()
+{
+    int dev = 0;
+    cudaDeviceProp prop;
+    return cudaGetDevice(&dev) == cudaSuccess && cudaGetDeviceProperties(&prop, dev) == cudaSuccess && prop.major == 10;
+}
+
+} // namespace
+
+extern "C" {
+
+int gw_probe_fp64_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, void *cuda_stream)
+{
+    if (n_iter < 1 || mode < 0 || mode > 5) return -1;
+    if (!arch_ok()) return -4;
+    return probe_fma_rate(n_iter, mode, fma_per_s, elapsed_ms, (cudaStream_t)cuda_stream) == cudaSuccess ? 0 : -3;
+}
+
+int gw_probe_store_bandwidth(int64_t bytes, int n_rep, double *gb_per_s, double *best_ms, void *cuda_stream)
+{
+    if (bytes < 16 || n_rep < 1) return -1;
+    if (!arch_ok()) return -4;
+    return probe_bandwidth(1, bytes, n_rep, gb_per_s, best_ms, (cudaStream_t)cuda_stream) == cudaSuccess ? 0 : -3;
+}
+
+int gw_probe_load_bandwidth(int64_t bytes, int n_rep, double *gb_per_s, double *best_ms, void *cuda_stream)
+{
+    if (bytes < 16 || n_rep < 1) return -1;
+    if (!arch_ok()) return -4;
+    return probe_bandwidth(0, bytes, n_rep, gb_per_s, best_ms, (cudaStream_t)cuda_stream) == cudaSuccess ? 0 : -3;
+}
+
+} // extern "C"

@@ -8,6 +8,7 @@ import numpy as np
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+COVERED_HEADERS = ("gwlnl.h", "gwlnl_tuning.h", "gwprobe.h")
 
 
 @pytest.fixture(scope="module")
@@ -18,8 +19,8 @@ def lib():
     return binding.load_library()
 
 
-def _declared_functions():
-    text = open(os.path.join(ROOT, "include", "gwlnl.h")).read()
+def _declared_functions(header="gwlnl.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(gw_[a-z0-9_]+)\s*\(", text)))
 
@@ -31,10 +32,32 @@ def test_header_symbols_are_exported(lib):
     for n in names:
         assert hasattr(lib, n), f"{n} declared in gwlnl.h but not exported"
     assert sorted(binding.EXPORTS) == names
+    tuning = _declared_functions("gwlnl_tuning.h")
+    assert sorted(binding.TUNING_EXPORTS) == tuning and tuning
+    for n in tuning:
+        assert hasattr(lib, n), f"{n} declared in gwlnl_tuning.h but not exported"
+    # the probes (fp64 rate, HBM bandwidth) live in their own library, not in the product library
+    assert not any(hasattr(lib, n) for n in _declared_functions("gwprobe.h"))
+
+
+def test_probe_library_exports_its_header():
+    from paper_1904_02863_b200.csrc import build as csrc_build
+    csrc_build.build_probe()
+    from paper_1904_02863_b200 import probes
+    plib = probes.load_library()
+    names = _declared_functions("gwprobe.h")
+    assert sorted(probes.EXPORTS) == names and names
+    for n in names:
+        assert hasattr(plib, n), f"{n} declared in gwprobe.h but not exported"
+
+
+def test_every_header_is_covered():
+    """Each header under include/ is checked against the library that implements it."""
+    assert sorted(os.listdir(os.path.join(ROOT, "include"))) == sorted(COVERED_HEADERS)
 
 
 def test_no_compute_calls(lib):
-    assert lib.gw_abi_version() == 3
+    assert lib.gw_abi_version() == 4
     assert lib.gw_strerror(0) == b"ok" and b"invalid" in lib.gw_strerror(-1)
     assert lib.gw_ctx_destroy(None) == 0
     assert lib.gw_ctx_info(None, None, None, None, None) == -1
@@ -77,6 +100,25 @@ def test_product_path_fails_loudly_without_gpu(lib):
     det = binding.detector_structs(np.array([[1, 0, 0, 0, 0, 0, 0, 0, 0, 0, 1, 0, 0.0]]))
     rc = lib.gw_ctx_create(ctypes.byref(h), f.size, f.ctypes.data, 1, d.ctypes.data, S.ctypes.data, det, 0.0, None, None)
     assert rc in (binding.GW_ERR_CUDA, binding.GW_ERR_ARCH) and not h
+
+
+def test_binding_rejects_bad_output_buffers():
+    """Caller-supplied outputs are validated before their raw pointers reach the library (no GPU needed: the checks
+    are static methods of the binding)."""
+    from paper_1904_02863_b200.binding import GwContext, GwError
+    for bad in (np.empty(7), np.empty(8, dtype=np.float32), np.empty((8, 2))[:, 0], [0.0] * 8):
+        with pytest.raises(GwError):
+            GwContext._out_host(bad, 8, "out")
+    ro = np.empty(8)
+    ro.flags.writeable = False
+    with pytest.raises(GwError):
+        GwContext._out_host(ro, 8, "out")
+    assert GwContext._out_host(np.empty(8), 8, "out") is not None
+    import torch
+    like = torch.empty(1)
+    for bad in (torch.empty(8), np.empty(8)):          # CPU tensor / not a tensor
+        with pytest.raises(GwError):
+            GwContext._out_dev(bad, 8, like, "out")
 
 
 def test_package_does_not_import_oracle():

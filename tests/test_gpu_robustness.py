@@ -6,7 +6,7 @@ import pytest
 
 from paper_1904_02863_b200 import inputs
 
-from gpu_common import assert_lnl_close, make_ctx, make_problem
+from gpu_common import assert_h_close, assert_lnl_close, make_ctx, make_problem
 
 pytestmark = pytest.mark.gpu
 
@@ -275,3 +275,56 @@ def test_tidal_outputs_stay_inside_their_buffers_and_theta_is_read_with_its_stri
             assert _intact(torch, lbuf, nl) and _intact(torch, pbuf, npart) and _intact(torch, hbuf, nh), B
             assert bool(torch.isfinite(lnl).all()) and bool(torch.isfinite(parts).all()) and bool(torch.isfinite(h).all()), B
         assert np.array_equal(ref_host, lnl.cpu().numpy())          # B = 600: host variant == device variant
+
+
+def test_first_call_on_a_non_blocking_stream_right_after_create_and_reserve(oracle):
+    """The workspace counters (cross-chunk tickets) are zeroed by create / reserve; a batch call issued at once on a
+    NON-BLOCKING stream (not ordered against the legacy default stream) must find them zeroed: multi-chunk plans,
+    one-level and two-level finish, straight after gw_ctx_create and straight after gw_ctx_reserve."""
+    import torch
+    from paper_1904_02863_b200 import binding
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=600.0, batch=700)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    ref = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th, cfg.spin_order)
+    stream = torch.cuda.Stream()                 # torch's pool streams are created with cudaStreamNonBlocking
+    thd = torch.from_numpy(th).cuda()
+    torch.cuda.synchronize()
+    for n_chunks in (7, 40):
+        for first in (300, 700):
+            ctx = binding.GwContext(f, d, S, dets, cfg.gmst, spin_order=cfg.spin_order, max_batch=first)
+            ctx.force_plan(1, n_chunks)
+            lnl, parts = ctx.lnl_batch(thd[:first].contiguous(), want_parts=True, stream=stream)
+            stream.synchronize()
+            assert_lnl_close(lnl.cpu().numpy(), parts.cpu().numpy(), ref[0][:first], ref[1][:first])
+            ctx.reserve(2 * first)                                              # new workspace, new counters
+            lnl, parts = ctx.lnl_batch(thd[:first].contiguous(), want_parts=True, stream=stream)
+            stream.synchronize()
+            assert_lnl_close(lnl.cpu().numpy(), parts.cpu().numpy(), ref[0][:first], ref[1][:first])
+            ctx.close()
+
+
+def test_large_fixed_delay_is_poisoned_not_garbled(oracle):
+    """A FIXED detector with a huge dt_s pushes f (t_c + dt) beyond the domain of the integer range reduction: the
+    outputs are NaN (boundary contract), while a moderate delay still matches the oracle."""
+    import torch
+    from paper_1904_02863_b200 import GwContext
+    f = 20.0 + np.arange(640) / 4.0
+    S = inputs.analytic_psd(f)[None].repeat(2, axis=0)
+    th = np.tile(np.array(inputs.CONFIGS["C0"].theta_inj), (4, 1))
+    th[:, inputs.P_TC] = [0.0, 0.05, -0.03, 0.01]
+    rng = np.random.Generator(np.random.PCG64(11))
+    d = (rng.standard_normal((2, f.size)) + 1j * rng.standard_normal((2, f.size))) * np.sqrt(S / (4 * 0.25))
+    for dt0, dt1, finite in ((0.3, -0.2, True), (4.0e6, 0.0, False), (0.0, 4.0e6, False)):
+        dets = np.stack([inputs.fixed_detector(1.0, 0.0, dt0), inputs.fixed_detector(0.3, -0.6, dt1)])
+        with GwContext(f, d, S, dets, 0.0, spin_order=0, max_batch=4) as ctx:
+            thd = torch.from_numpy(th).cuda()
+            lnl, parts = ctx.lnl_batch(thd, want_parts=True)
+            h = ctx.waveform_batch(thd)
+            torch.cuda.synchronize()
+            lnl, parts, h = lnl.cpu().numpy(), parts.cpu().numpy(), h.cpu().numpy()
+        if finite:
+            ref = oracle.lnl(f, 0.25, d, S, dets, 0.0, th, 0)
+            assert_lnl_close(lnl, parts, ref[0], ref[1])
+            assert_h_close(h, oracle.waveform(f, dets, 0.0, th, 0))
+        else:
+            assert np.all(np.isnan(lnl)) and np.all(np.isnan(h))
