@@ -231,6 +231,8 @@ def run_ours(args):
     ctx = GwContext(f, d, S, dets, cfg.gmst, spin_order=cfg.spin_order, max_batch=B,
                     isco_cut=int(args.isco_cut), phase_marginal=int(args.phase_marginal),
                     tidal_order=int(args.tidal_order))
+    if args.force_grid or args.force_lpp:                 # tuning aid (include/gwlnl_tuning.h): pin the launch shape
+        ctx.force_grid(args.force_lpp, args.force_grid)
     thd = torch.from_numpy(th).cuda()
     lnl = torch.empty(B, dtype=torch.float64, device="cuda")
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
@@ -268,6 +270,7 @@ def run_ours(args):
             ev0[i].record(stream)
             step()
             ev1[i].record(stream)
+        clock_after_mhz = probes.sm_clock_mhz()      # the clock the timed kernels actually ran at (enqueued right behind them)
         torch.cuda.synchronize()
     launches = ctx.launch_count() - launches0
     if world > 1:
@@ -406,6 +409,9 @@ def run_ours(args):
         cpu["single_thread"] = {"value": r1, "cores": u1, "sample": f"first {n1} proposals x {p1} passes, {dt1:.1f} s wall"}
 
     clocks = clk.summary()
+    clocks["sm_mhz_measured_after_timed_region"] = clock_after_mhz
+    clocks["note"] = ("sm_mhz: NVML samples during the timed region (the requested clock); sm_mhz_measured_after_timed_region: "
+                      "clock64 against globaltimer in a probe kernel enqueued right behind the last timed step")
     ctx.close()
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n_gpus, "steps": args.steps,
@@ -416,6 +422,7 @@ def run_ours(args):
                 "config": {"workload": f"{name}: {n_det} det x {M} bins x {B} proposals per GPU",
                            "global_batch": B * world, "bins": M, "detectors": n_det, "parallelism": f"proposals sharded x{world}",
                            "l2": "flushed before every timed step: 256 MiB write, then a 256 MiB read of a second buffer (no dirty lines left)", "plan": plan,
+                           "pinned": {"grid": args.force_grid, "lanes_per_prop": args.force_lpp},
                            "options": {"isco_cut": int(args.isco_cut), "phase_marginal": int(args.phase_marginal),
                                        "tidal_order": int(args.tidal_order)}},
                 "bin_det_proposals_per_s": value * M * n_det,
@@ -437,6 +444,8 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-waveform", action="store_true")
+    ap.add_argument("--force-grid", type=int, default=0, help="tuning aid: pin the fused kernel's grid to this many CTAs")
+    ap.add_argument("--force-lpp", type=int, default=0, help="tuning aid: pin the lanes per proposal (1, 2, ..., 32)")
     ap.add_argument("--isco-cut", action="store_true", help="NEXT-1 option: h = 0 above f_ISCO (not the headline config)")
     ap.add_argument("--phase-marginal", action="store_true", help="NEXT-1 option: lnL marginalised over phi_c")
     ap.add_argument("--tidal-order", type=int, default=0, choices=[0, 1, 2],

@@ -18,6 +18,16 @@ extern "C" {
  * fit the reserved workspace makes gw_lnl_batch return GW_ERR_INVALID_ARG.                              */
 int gw_ctx_force_plan(gw_ctx *ctx, int lanes_per_prop, int n_chunks);
 
+/* Testing / tuning aid: pin the grid instead -- n_ctas CTAs share the flattened (proposal tile, bin) space equally,
+ * whatever the tile count (n_ctas >= 1; 0 leaves the choice to the planner; overrides a pinned n_chunks).       */
+int gw_ctx_force_grid(gw_ctx *ctx, int lanes_per_prop, int64_t n_ctas);
+
+/* Host-only (no CUDA call): the segments that CTA `cta` of a grid of n_ctas CTAs sweeps when n_tiles proposal tiles
+ * of n_bins bins are shared equally -- the same arithmetic the fused kernel runs (csrc/gw_internal.h, segment_at).
+ * Writes up to max_rows rows of 6 values (tile, j0, j1, index of the segment within its tile, segments of that tile,
+ * partial-sum slot) and returns the number of segments of the CTA, or GW_ERR_INVALID_ARG.                     */
+int gw_plan_cta_segments(int64_t n_tiles, int64_t n_bins, int64_t n_ctas, int64_t cta, int max_rows, int64_t *rows6);
+
 /* Measurement aid: when enabled, the *_batch calls record CUDA events on their stream before the setup
  * kernel, between the setup kernel and the main (fused or waveform) kernel, and after it.  The event between
  * the two launches removes their programmatic overlap, so enable it only for kernel-level timing.

@@ -25,6 +25,12 @@ extern "C" {
  * 4, 5 = mode 0 with 8 or 16 independent integer instructions beside every 8 DFMA.                        */
 int gw_probe_fp64_fma_rate(int n_iter, int mode, double *fma_per_s, double *elapsed_ms, void *cuda_stream);
 
+/* The SM clock that is actually running, in MHz (median over the SMs): one warp per SM spins for ~30 us of clock64()
+ * between two reads of the nanosecond globaltimer.  Enqueued on `cuda_stream` right behind the timed work, it shows the
+ * clock the preceding kernels ran at (NVML reports the requested clock; power management adjusts on a millisecond
+ * scale).                                                                                                    */
+int gw_probe_sm_clock(double *mhz_median, void *cuda_stream);
+
 /* Pure-store HBM bandwidth: `bytes` (far larger than the 126 MB L2) written once per pass with 16-byte streaming
  * stores by a grid of 8 CTAs per SM; best of `n_rep` passes after one warm-up pass.  GB/s = bytes / best time.   */
 int gw_probe_store_bandwidth(int64_t bytes, int n_rep, double *gb_per_s, double *best_ms, void *cuda_stream);

@@ -27,7 +27,8 @@ EXPORTS = (
     "gw_ctx_launch_count", "gw_strerror", "gw_last_cuda_error", "gw_abi_version",
 )
 # include/gwlnl_tuning.h: testing / tuning aids exported by the same library, outside the product boundary
-TUNING_EXPORTS = ("gw_ctx_force_plan", "gw_ctx_kernel_timing", "gw_ctx_last_kernel_ms")
+TUNING_EXPORTS = ("gw_ctx_force_plan", "gw_ctx_force_grid", "gw_plan_cta_segments", "gw_ctx_kernel_timing",
+                  "gw_ctx_last_kernel_ms")
 
 
 class GwError(RuntimeError):
@@ -82,6 +83,8 @@ def load_library():
     lib.gw_ctx_launch_count.argtypes = [vp]
     lib.gw_ctx_launch_count.restype = i64
     lib.gw_ctx_force_plan.argtypes = [vp, ci, ci]
+    lib.gw_ctx_force_grid.argtypes = [vp, ci, i64]
+    lib.gw_plan_cta_segments.argtypes = [i64, i64, i64, i64, ci, P(i64)]
     lib.gw_ctx_kernel_timing.argtypes = [vp, ci]
     lib.gw_ctx_last_kernel_ms.argtypes = [vp, P(dbl), P(dbl)]
     lib.gw_strerror.argtypes = [ci]
@@ -220,6 +223,10 @@ class GwContext:
         """Pin the launch shape of lnl_batch (0 = planner's choice); a testing / tuning aid."""
         _check(self._lib.gw_ctx_force_plan(self._h, int(lanes_per_prop), int(n_chunks)), "gw_ctx_force_plan", self._h)
 
+    def force_grid(self, lanes_per_prop: int = 0, n_ctas: int = 0):
+        """Pin the grid of lnl_batch: n_ctas CTAs share the (tile, bin) space equally (0 = planner's choice)."""
+        _check(self._lib.gw_ctx_force_grid(self._h, int(lanes_per_prop), int(n_ctas)), "gw_ctx_force_grid", self._h)
+
     def kernel_timing(self, enable: bool):
         _check(self._lib.gw_ctx_kernel_timing(self._h, int(bool(enable))), "gw_ctx_kernel_timing", self._h)
 
@@ -321,6 +328,19 @@ class GwContext:
         rc = self._lib.gw_waveform_batch_host(self._h, n, _host_ptr(th), _host_ptr(out), _stream_ptr(stream))
         _check(rc, "gw_waveform_batch_host", self._h)
         return out
+
+
+def plan_cta_segments(n_tiles: int, n_bins: int, n_ctas: int, cta: int, max_rows: int = 64) -> np.ndarray:
+    """gw_plan_cta_segments (host only): rows (tile, j0, j1, index, count, slot) of the segments one CTA sweeps."""
+    lib = load_library()
+    rows = np.zeros((max_rows, 6), dtype=np.int64)
+    n = lib.gw_plan_cta_segments(int(n_tiles), int(n_bins), int(n_ctas), int(cta), int(max_rows),
+                                 rows.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)))
+    if n < 0:
+        raise GwError(n, "gw_plan_cta_segments", "invalid argument")
+    if n > max_rows:
+        return plan_cta_segments(n_tiles, n_bins, n_ctas, cta, n)
+    return rows[:n]
 
 
 def waveform_for_inputs(freqs, det_rows, gmst, theta, spin_order):

@@ -24,6 +24,7 @@ struct gw_ctx {
     int          last_cuda_error;
     int64_t      launches;
     int          force_lpp, force_chunks;   // gw_ctx_force_plan (0 = planner's choice)
+    int64_t      force_ctas;       // gw_ctx_force_grid (0 = planner's choice)
     int64_t      plan_n[4];        // batch sizes of the cached plans (0 = empty): a sampler calls with few distinct sizes
     Plan         plan_of[4];       // make_plan is a pure function of n_prop for a given context and pinned shape
     int          plan_next;
@@ -92,18 +93,32 @@ constexpr double kMultiPenalty = GW_MULTI_PENALTY;     // the lanes-interleaved 
 constexpr double kTwoLevelHop = 16.0;      // the second fence + ticket round of the two-level finish (~2 us; C4 B = 1, 16)
 constexpr double kFinishPerChunk = 1.0;    // serial additions of the finish stage, in bin-sweep equivalents each (calibrated on C4 B = 256, 512)
 
+// exact maximum of segments per tile for a grid of n_cta CTAs over n_tiles tiles of M bins
+int max_segments_per_tile(int64_t n_tiles, int64_t M, int64_t n_cta)
+{
+    const int64_t work = n_tiles * M;
+    if (n_cta % n_tiles == 0) return (int)(n_cta / n_tiles);           // aligned grid: every tile in n_cta / n_tiles chunks
+    int64_t best = 1;
+    for (int64_t t = 0; t < n_tiles; ++t) {
+        const int64_t c = cta_of_position(t * M + M - 1, work, n_cta) - cta_of_position(t * M, work, n_cta) + 1;
+        if (c > best) best = c;
+    }
+    return (int)best;
+}
+
 Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
 {
     const int64_t M = ctx->t.n_bins;
     const int slots_per_sm = ctx->ctas_per_sm > 0 ? ctx->ctas_per_sm : 1;
     const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 148;
     const int64_t slots = (int64_t)n_sm * slots_per_sm;
-    Plan best = {1, kThreads, 1, (n_prop + kThreads - 1) / kThreads, 1, 0};
+    Plan best = {1, kThreads, (n_prop + kThreads - 1) / kThreads, (n_prop + kThreads - 1) / kThreads, 1, 1, 0};
     double best_cost = 1e300;
     for (int lpp = 1; lpp <= 32; lpp *= 2) {
         if (ctx->force_lpp > 0 && lpp != ctx->force_lpp) continue;
         const int pt = kThreads / lpp;
         const int64_t tiles = (n_prop + pt - 1) / pt;
+        const int64_t work = tiles * M;
         int64_t max_chunks = M / ((int64_t)8 * lpp);          // at least 8 iterations per thread
         const int64_t by_waves = (kMaxWaves * slots) / tiles; // no more than kMaxWaves waves of CTAs
         if (max_chunks > by_waves) max_chunks = by_waves;
@@ -111,32 +126,52 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
         if (max_chunks < 1) max_chunks = 1;
         int64_t nc_first = 1;
         if (ctx->force_chunks > 0) { nc_first = max_chunks = (ctx->force_chunks < M ? ctx->force_chunks : M); }
-        for (int64_t nc = nc_first; nc <= max_chunks; ++nc) {
-            const int64_t ctas = tiles * nc;
-            const int64_t chunk = (M + nc - 1) / nc;
-            const double sweep = (double)((chunk + lpp - 1) / lpp) * (lpp > 1 ? kMultiPenalty : 1.0);
-            const double pro = kProBins + (lpp > 1 ? 2.0 : 0.0);
+        // candidate grids: the aligned ones (every tile in nc equal chunks), and -- unless a shape is pinned -- the two
+        // balanced ones (one or all resident CTAs per SM, whatever the tile count)
+        int64_t n_aligned = max_chunks - nc_first + 1;
+        int64_t n_cand = n_aligned + (ctx->force_chunks > 0 ? 0 : 2);
+        if (ctx->force_ctas > 0) { n_aligned = 0; n_cand = 1; }                 // a pinned grid is the only candidate
+        for (int64_t ci = 0; ci < n_cand; ++ci) {
+            int64_t ctas;
+            bool aligned = ci < n_aligned;
+            if (ctx->force_ctas > 0) {
+                ctas = ctx->force_ctas < work ? ctx->force_ctas : work;
+                aligned = ctas % tiles == 0;
+            } else if (aligned) ctas = tiles * (nc_first + ci);
+            else {
+                ctas = (ci == n_aligned) ? n_sm : slots;
+                if (ctas % tiles == 0) continue;                                // already among the aligned grids
+                if (work / ctas < (int64_t)8 * lpp) continue;                    // at least 8 iterations per thread
+            }
+            const double bins_per_cta = (double)work / (double)ctas;
+            const double sweep = std::ceil(bins_per_cta / lpp) * (lpp > 1 ? kMultiPenalty : 1.0);
+            // segments a CTA sweeps: one, plus one per tile boundary inside its range (each costs a prologue / epilogue)
+            const double segs = aligned ? 1.0 : 1.0 + std::fmin(1.0, (double)(tiles - 1) / (double)ctas) + std::floor(bins_per_cta / (double)M);
+            const double pro = (kProBins + (lpp > 1 ? 2.0 : 0.0)) * segs;
             const int64_t per_sm = (ctas + n_sm - 1) / n_sm;                  // CTAs an SM must run
             const int64_t waves = (per_sm + slots_per_sm - 1) / slots_per_sm;
             const double resident = (double)per_sm / (double)waves;           // average co-resident CTAs
             const double warps_per_sched = resident * (kThreads / 32) / 4.0;
             double slowdown = warps_per_sched > kSatWarps ? warps_per_sched / kSatWarps : 1.0;
             if (resident >= 2.0) slowdown *= (lpp > 1 ? kCoResidentGainMulti : kCoResidentGain);  // a second CTA hides the first one's stage boundaries
-            const double finish_len = nc >= kFinishTwoLevelFrom ? kTwoLevelHop + (double)(kFinishGroup + (nc + kFinishGroup - 1) / kFinishGroup)
-                                                                : (double)nc;   // serial additions of the finish
+            const int64_t nseg = aligned ? ctas / tiles : (ctas + tiles - 1) / tiles + 1;   // segments per tile
+            const double finish_len = nseg >= kFinishTwoLevelFrom ? kTwoLevelHop + (double)(kFinishGroup + (nseg + kFinishGroup - 1) / kFinishGroup)
+                                                                  : (double)nseg;   // serial additions of the finish
             // lanes-interleaved CTAs have short sweeps and a latency-bound prologue that a co-resident CTA covers
             const double per_cta = lpp > 1 ? sweep * slowdown + pro : (sweep + pro) * slowdown;
+            // SMs that run one CTA more than the others set the time of an unbalanced grid
             const double cost = (double)waves * per_cta + kFinishPerChunk * finish_len;
             if (cost < best_cost) {
                 best_cost = cost;
-                best.lpp = lpp; best.props_per_cta = pt; best.n_chunks = (int)nc; best.n_tiles = tiles;
+                best.lpp = lpp; best.props_per_cta = pt; best.n_cta = ctas; best.n_tiles = tiles;
                 // a grid that fits one CTA per SM is launched so that no SM takes two (launch_fused)
                 best.exclusive = (GW_EXCLUSIVE_PLANS && ctas <= n_sm) ? 1 : 0;
             }
         }
         if (tiles >= slots && ctx->force_lpp == 0) break;     // enough proposals to fill the GPU: keep this lpp
     }
-    best.n_groups = best.n_chunks >= kFinishTwoLevelFrom ? (best.n_chunks + kFinishGroup - 1) / kFinishGroup : 1;
+    best.max_seg = max_segments_per_tile(best.n_tiles, M, best.n_cta);
+    best.gmax = best.max_seg >= kFinishTwoLevelFrom ? (best.max_seg + kFinishGroup - 1) / kFinishGroup : 1;
     return best;
 }
 
@@ -158,13 +193,13 @@ int64_t partial_bound(const gw_ctx *ctx, int64_t max_batch)
 {
     const int slots_per_sm = ctx->ctas_per_sm > 0 ? ctx->ctas_per_sm : 1;
     const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 148;
-    const int64_t ctas = kMaxWaves * (int64_t)n_sm * slots_per_sm + (max_batch + kThreads - 1) / kThreads + 1;
+    const int64_t ctas = kMaxWaves * (int64_t)n_sm * slots_per_sm + 2 * ((max_batch + kThreads - 1) / kThreads) + 4;   // n_cta + n_tiles slots
     return ctas * kThreads * (int64_t)(2 * ctx->t.n_det);
 }
 
 int64_t partial_need(const gw_ctx *ctx, const Plan &p)
 {
-    return p.n_chunks > 1 ? p.n_tiles * p.n_chunks * (int64_t)(2 * ctx->t.n_det) * p.props_per_cta : 0;
+    return p.max_seg > 1 ? plan_partial_slots(p) * (int64_t)(2 * ctx->t.n_det) * p.props_per_cta : 0;
 }
 
 void free_workspace(Workspace &w)
@@ -418,8 +453,8 @@ int gw_ctx_plan(const gw_ctx *ctx, int64_t n_prop, int *lanes_per_prop, int *pro
     const Plan p = make_plan(ctx, n_prop);
     if (lanes_per_prop) *lanes_per_prop = p.lpp;
     if (props_per_cta) *props_per_cta = p.props_per_cta;
-    if (n_chunks) *n_chunks = p.n_chunks;
-    if (n_ctas) *n_ctas = p.n_tiles * p.n_chunks;
+    if (n_chunks) *n_chunks = p.max_seg;
+    if (n_ctas) *n_ctas = p.n_cta;
     return GW_OK;
 }
 
@@ -430,8 +465,40 @@ int gw_ctx_force_plan(gw_ctx *ctx, int lanes_per_prop, int n_chunks)
         return GW_ERR_INVALID_ARG;
     ctx->force_lpp = lanes_per_prop;
     ctx->force_chunks = n_chunks;
+    ctx->force_ctas = 0;
     for (int i = 0; i < 4; ++i) ctx->plan_n[i] = 0;          // cached plans were made for the previous pin
     return GW_OK;
+}
+
+int gw_ctx_force_grid(gw_ctx *ctx, int lanes_per_prop, int64_t n_ctas)
+{
+    if (!ctx || n_ctas < 0 || n_ctas > 0x7fffffffLL) return GW_ERR_INVALID_ARG;
+    if (lanes_per_prop != 0 && (lanes_per_prop < 1 || lanes_per_prop > 32 || (lanes_per_prop & (lanes_per_prop - 1)) != 0))
+        return GW_ERR_INVALID_ARG;
+    ctx->force_lpp = lanes_per_prop;
+    ctx->force_chunks = 0;
+    ctx->force_ctas = n_ctas;
+    for (int i = 0; i < 4; ++i) ctx->plan_n[i] = 0;
+    return GW_OK;
+}
+
+int gw_plan_cta_segments(int64_t n_tiles, int64_t n_bins, int64_t n_ctas, int64_t cta, int max_rows, int64_t *rows6)
+{
+    if (n_tiles < 1 || n_bins < 1 || n_ctas < 1 || cta < 0 || cta >= n_ctas || max_rows < 0 || (max_rows > 0 && !rows6))
+        return GW_ERR_INVALID_ARG;
+    if ((double)n_tiles * (double)n_bins * (double)(n_ctas + 1) > 4.0e18) return GW_ERR_INVALID_ARG;
+    const int64_t work = n_tiles * n_bins;
+    const int64_t w_end = work_begin(cta + 1, work, n_ctas);
+    int n = 0;
+    for (int64_t w = work_begin(cta, work, n_ctas); w < w_end; ++n) {
+        const Segment s = segment_at(w, w_end, cta, n_bins, work, n_ctas);
+        if (n < max_rows) {
+            int64_t *r = rows6 + 6 * n;
+            r[0] = s.tile; r[1] = s.j0; r[2] = s.j1; r[3] = s.index; r[4] = s.count; r[5] = s.slot;
+        }
+        w += s.j1 - s.j0;
+    }
+    return n;
 }
 
 int gw_ctx_norms(const gw_ctx *ctx, double *i7_host)
@@ -479,9 +546,10 @@ static int lnl_batch_impl(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, 
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const Plan p = cached_plan(ctx, n_prop);
     if (partial_need(ctx, p) > ctx->w.partial_doubles || p.n_tiles > ctx->w.n_tickets) return GW_ERR_INVALID_ARG;
-    if (p.n_groups > 1 && (p.n_tiles * p.n_groups * (int64_t)(2 * ctx->t.n_det) * p.props_per_cta > ctx->w.gpartial_doubles ||
-                           p.n_tiles * p.n_groups > ctx->w.n_gtickets))
+    if (p.gmax > 1 && (p.n_tiles * p.gmax * (int64_t)(2 * ctx->t.n_det) * p.props_per_cta > ctx->w.gpartial_doubles ||
+                       p.n_tiles * p.gmax > ctx->w.n_gtickets))
         return GW_ERR_INVALID_ARG;
+    if ((double)p.n_tiles * (double)ctx->t.n_bins * (double)(p.n_cta + 1) > 4.0e18) return GW_ERR_INVALID_ARG;   // 64-bit range arithmetic
     if (ctx->timing) cudaEventRecord(ctx->ev[0], s);
     cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
                                  ctx->w.rec_stride, (double)p.lpp * ctx->t.delta_f, 1, theta_in_host_memory, s,

@@ -76,14 +76,53 @@ struct Tables {
 };
 
 // Launch shape of one gw_lnl_batch call (a pure function of n_prop and the context; fixes summation order).
+// The (tile, bin) pairs of a call form one flattened space of work = n_tiles * n_bins positions, tile-major; CTA k of
+// n_cta sweeps the contiguous range [k work / n_cta, (k+1) work / n_cta).  Where a range crosses a tile boundary the
+// CTA sweeps two (or more) SEGMENTS, one per tile; a tile's segments are summed in ascending bin order.  With
+// n_cta = n_tiles * n_chunks the ranges are the n_chunks equal chunks of every tile (the round-1 shape, and what
+// gw_ctx_force_plan pins); with n_cta = SMs x resident CTAs every CTA gets the same number of bins whatever the
+// shape -- no idle SMs, no second partial wave.
 struct Plan {
     int     lpp;          // lanes per proposal (1,2,4,...,32)
     int     props_per_cta;// kThreads / lpp
-    int     n_chunks;     // frequency chunks per proposal tile
     int64_t n_tiles;      // ceil(n_prop / props_per_cta)
-    int     n_groups;     // 1, or ceil(n_chunks / kFinishGroup) when the finish is two-level
+    int64_t n_cta;        // CTAs of the grid
+    int     max_seg;      // upper bound of segments per tile (what gw_ctx_plan reports as n_chunks)
+    int     gmax;         // groups per tile of the two-level finish: stride of the group workspace (>= 1)
     int     exclusive;    // 1: the grid has at most one CTA per SM and is launched so that no SM takes two
 };
+
+// ---- flattened work ranges (shared by the kernel, the planner and the CPU tests of the host logic) --------------
+// first flattened position of CTA k
+__host__ __device__ inline int64_t work_begin(int64_t k, int64_t work, int64_t n_cta) { return (k * work) / n_cta; }
+// the CTA whose range holds flattened position p: the largest k with floor(k work / n_cta) <= p
+__host__ __device__ inline int64_t cta_of_position(int64_t p, int64_t work, int64_t n_cta)
+{
+    return ((p + 1) * n_cta + work - 1) / work - 1;
+}
+// One segment = the part of a CTA's range that lies in one tile.
+struct Segment {
+    int64_t tile, j0, j1;  // bins [j0, j1) of proposal tile `tile`
+    int64_t first_cta;     // the CTA that holds the tile's first bin
+    int     index;         // position among the tile's segments (ascending bins) = cta - first_cta
+    int     count;         // segments of the tile
+    int64_t slot;          // partial-sum slot = cta + tile: consecutive along a tile, unique over the grid
+};
+__host__ __device__ inline Segment segment_at(int64_t w, int64_t w_end, int64_t cta, int64_t n_bins, int64_t work,
+                                              int64_t n_cta)
+{
+    Segment s;
+    s.tile = w / n_bins;
+    s.j0 = w - s.tile * n_bins;
+    const int64_t left = w_end - w;
+    s.j1 = (n_bins - s.j0 < left) ? n_bins : s.j0 + left;
+    s.first_cta = cta_of_position(s.tile * n_bins, work, n_cta);
+    const int64_t last_cta = cta_of_position(s.tile * n_bins + n_bins - 1, work, n_cta);
+    s.index = (int)(cta - s.first_cta);
+    s.count = (int)(last_cta - s.first_cta + 1);
+    s.slot = cta + s.tile;
+    return s;
+}
 
 struct Workspace {
     int64_t max_batch;    // reserved proposals
@@ -113,6 +152,8 @@ cudaError_t launch_setup(const Tables &t, const DetSet &dets, double gmst, int s
 cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, const double *rec,
                          int64_t rec_stride, double *partial, unsigned int *tickets, double *gpartial,
                          unsigned int *gtickets, double *lnl_out, double *parts_out, cudaStream_t s, int64_t *launches);
+// chunk partial sums: one slot of 2 n_det props_per_cta doubles per segment
+inline int64_t plan_partial_slots(const Plan &p) { return p.n_cta + p.n_tiles; }
 cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, int64_t rec_stride,
                             double *h_out, cudaStream_t s, int64_t *launches);
 cudaError_t configure_kernels(int *fused_ctas_per_sm);      // smem attributes + occupancy query (per n_det below)

@@ -562,31 +562,36 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
 // =====================================================================================================
 // K3: fused waveform + projection + inner product (north_star item (4); steps a2..a5)
 //
-// CTA = kThreads threads = (kThreads / lpp) proposals x one chunk of frequency bins [j0, j1).
+// The (proposal tile, bin) pairs of a call form one flattened space, tile-major; CTA k of n_cta sweeps the contiguous
+// range [k work / n_cta, (k+1) work / n_cta) of it (gw_internal.h, struct Plan): one SEGMENT per tile the range touches,
+// i.e. kThreads threads = (kThreads / lpp) proposals x the bins [j0, j1) of that tile.  Every CTA gets the same number of
+// bins whatever the batch size, so no SM idles and no partial second wave exists.
 // lpp = lanes per proposal: 1 for sampler-sized batches (each thread owns one proposal and sweeps the
 // chunk; the tables are read from shared memory as warp broadcasts), 2..32 for small batches (the lanes
 // of a proposal interleave over the bins; a fixed xor-shuffle tree combines them).
-// The chunk is streamed through a kStages-deep ring of kStageBins-bin stages by bulk async copies (TMA
+// A segment is streamed through a kStages-deep ring of kStageBins-bin stages by bulk async copies (TMA
 // engine) completing on mbarriers.  Per (proposal, bin): 9 FMA phase (incl. f tau_0), 12-op sincos (cis_phase_lnl) giving
 // E = e^{+2 pi i (Phi' + f tau_0)}, detector 0: Z_0 += g_0j E (4 FMA), and per detector I >= 1
 //     Z_I <- Z_I * rot_I + g_Ij * E                                                  (8 fp64 ops)
 // where rot_I = exp(-2 pi i lpp df (tau_I - tau_0)): after the sweep Z_I * exp(+2 pi i f_last (tau_I - tau_0))
 // equals sum_j g_Ij exp(+2 pi i (Phi'_j + f_j tau_I)), i.e. the time shift of PAPER.md:69 costs no sincos.
 // <h|h>_I = |CA_I|^2 I7_I exactly for this waveform, so only <d|h> is accumulated.
-// Cross-chunk: partials to the workspace, a per-tile ticket, and the last CTA of a tile sums the chunks in
-// index order (deterministic) and writes lnL and parts.
+// Cross-segment: partials to the workspace, a per-tile ticket, and the last CTA of a tile sums the tile's segments in
+// ascending bin order (deterministic: the order is a function of (n_tiles, n_bins, n_cta) alone) and writes lnL and parts.
 // =====================================================================================================
 struct FusedArgs {
     const double *planes, *rec;
     int64_t n_pad, n_bins, n_prop, rec_stride;
-    int     n_chunks, lpp;
+    int64_t work;            // n_tiles * n_bins: size of the flattened (tile, bin) space
+    int64_t n_cta;           // CTAs of the grid: CTA k sweeps [k work / n_cta, (k+1) work / n_cta)
+    int     lpp;
+    int     gmax;            // groups per tile of the two-level finish (stride of gpartial / gtickets)
     double  f0, delta_f;
     double  i7[GW_MAX_DET];
     const double *i7cum;     // isco_cut: [NDET][n_pad] prefix sums of the norm
     int     phase_marginal;
-    double *partial;
-    unsigned int *tickets;
-    int     n_groups;        // > 1: two-level finish over groups of kFinishGroup chunks
+    double *partial;         // [slot][2 NDET][PT] segment sums, slot = cta + tile
+    unsigned int *tickets;   // [tile]
     double *gpartial;        // [tile][group][2 NDET][PT] group sums
     unsigned int *gtickets;  // [tile][group]
     double *lnl, *parts;
@@ -647,34 +652,35 @@ __device__ __forceinline__ void finish_proposal(const FusedArgs &a, int64_t b, c
     a.lnl[b] = lnl;
 }
 
+// One segment: bins [seg.j0, seg.j1) of proposal tile seg.tile.  `g` is the CTA's running position in the stage ring
+// (stages issued so far): stage s of the segment uses buffer (g + s) % kStages and completes phase (g + s) / kStages of
+// its mbarrier, so the ring carries on from segment to segment without re-initialisation.
 template <int NDET, bool MULTI, bool ISCO, bool TIDAL>
-__global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedArgs a)
+__device__ __forceinline__ void fused_segment(const FusedArgs &a, const Segment &seg, uint32_t &g, const bool first,
+                                              unsigned char *smem_raw, unsigned int &s_ticket, int &s_relmax)
 {
     constexpr int NP = kBasisPlanes + NDET;                  // planes per stage
-    extern __shared__ __align__(128) unsigned char smem_raw[];
     double2  *sm   = reinterpret_cast<double2 *>(smem_raw);
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + (size_t)kStages * NP * kStageBins * sizeof(double2));
-    __shared__ unsigned int s_ticket;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int lpp = MULTI ? a.lpp : 1;
     const int ppw = 32 / lpp;
     const int PT  = kThreads / lpp;
-    const int chunk = blockIdx.x % a.n_chunks;
-    const int64_t tile = blockIdx.x / a.n_chunks;
+    const int64_t tile = seg.tile;
     const int pic = MULTI ? warp * ppw + lane / lpp : tid;   // proposal slot in this CTA
     const int sub = MULTI ? lane % lpp : 0;                  // lane's position among the proposal's lanes
     int64_t b = tile * PT + pic;
     const bool live = b < a.n_prop;
     if (!live) b = a.n_prop - 1;
 
-    const int64_t j0 = ((int64_t)chunk * a.n_bins) / a.n_chunks;
-    const int64_t j1 = ((int64_t)(chunk + 1) * a.n_bins) / a.n_chunks;
-    const int n = (int)(j1 - j0);
+    const int64_t j0 = seg.j0;
+    const int n = (int)(seg.j1 - seg.j0);
     const int n_stage = (n + kStageBins - 1) / kStageBins;
+    const int n_issued0 = min(kStages, n_stage);             // stages prefetched before the records are known
 
     auto issue_stage = [&](int s) {
-        const int buf = s % kStages;
+        const int buf = (int)((g + (uint32_t)s) % kStages);
         const int cnt = min(kStageBins, n - s * kStageBins);
         const uint32_t bytes = (uint32_t)cnt * (uint32_t)sizeof(double2);
         mbar_arrive_expect_tx(&bars[buf], bytes * NP);
@@ -684,17 +690,11 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             bulk_g2s(sm + (size_t)(buf * NP + p) * kStageBins, src + (int64_t)p * a.n_pad, bytes, &bars[buf]);
     };
 
-    __shared__ int s_relmax;
     if (tid == 0) {
-        for (int s = 0; s < kStages; ++s) mbar_init(&bars[s], 1);
-        mbar_fence_init();
-        s_relmax = -1;
+        if (ISCO) s_relmax = -1;
+        for (int s = 0; s < n_issued0; ++s) issue_stage(s);   // tables do not depend on K1
     }
-    __syncthreads();
-    if (tid == 0)
-        for (int s = 0; s < kStages && s < n_stage; ++s) issue_stage(s);   // tables do not depend on K1
-
-    pdl_wait_primary();                                      // records come from the setup kernel
+    if (first) pdl_wait_primary();                           // records come from the setup kernel
     const PhaseCoef k = load_coef(a.rec, a.rec_stride, b);
     double t10 = 0.0, t12 = 0.0;                             // NEXT-1 option: tidal terms t10 x^5 + t12 x^7
     if (TIDAL) {
@@ -711,34 +711,38 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
         zr[i] = 0.0; zi[i] = 0.0;
     }
 
-    int64_t jcut = 0;
-    int n_run = n_stage;                                     // stages this CTA sweeps
+    int jrel = 0;                                            // isco_cut: last kept bin relative to j0 (may be < 0 or >= n)
+    int n_run = n_stage;                                     // stages this segment sweeps
+    int n_issued = n_stage;                                  // stages whose copies are issued (>= n_run)
     if (ISCO) {
         // Stages wholly above the cut-off of every proposal of the CTA contribute nothing: they are neither loaded
         // (beyond the prefetched ones) nor swept.  The rotation recurrence stops with the last swept bin, which is
         // the f_last of the seed below.
-        jcut = (int64_t)a.rec[(int64_t)rec_field_jcut(NDET) * a.rec_stride + b];
-        int rel = (int)max((int64_t)-1, min(jcut - j0, (int64_t)n - 1));
+        const int64_t jcut = (int64_t)a.rec[(int64_t)rec_field_jcut(NDET) * a.rec_stride + b];
+        jrel = (int)max((int64_t)-1, min(jcut - j0, (int64_t)n));
+        int rel = min(jrel, n - 1);
         rel = __reduce_max_sync(0xffffffffu, rel);
+        __syncthreads();                                     // s_relmax = -1 of this segment is in place
         if (lane == 0) atomicMax(&s_relmax, rel);
         __syncthreads();
         n_run = s_relmax < 0 ? 0 : s_relmax / kStageBins + 1;
+        n_issued = max(n_run, n_issued0);
     }
     int iters_total = 0;
     for (int s = 0; s < n_stage; ++s) {
-        const int buf = s % kStages;
+        const int buf = (int)((g + (uint32_t)s) % kStages);
+        const uint32_t parity = ((g + (uint32_t)s) / kStages) & 1u;
         const int cnt = min(kStageBins, n - s * kStageBins);
         if (ISCO && s >= n_run) {                            // drain the prefetched stages, then stop
-            if (s >= kStages) break;
-            mbar_wait(&bars[buf], 0u);
+            if (s >= n_issued) break;
+            mbar_wait(&bars[buf], parity);
             continue;
         }
-        mbar_wait(&bars[buf], (uint32_t)((s / kStages) & 1));
+        mbar_wait(&bars[buf], parity);
         const double2 *P = sm + (size_t)buf * NP * kStageBins;
         const int iters = MULTI ? (cnt + lpp - 1) / lpp : cnt;
-        const int64_t jstage = j0 + (int64_t)s * kStageBins;  // global index of the stage's first bin
         // last kept bin of this proposal relative to the stage (isco_cut), in [-1, kStageBins]
-        const int cut_local = ISCO ? (int)max((int64_t)-1, min(jcut - jstage, (int64_t)kStageBins)) : 0;
+        const int cut_local = ISCO ? max(-1, min(jrel - s * kStageBins, kStageBins)) : 0;
         int it = 0;
         if (!MULTI) {
             // kUnroll bins per trip, written plane by plane ("k-major"): consecutive fp64 instructions then
@@ -883,7 +887,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
         }
         iters_total += iters;
         __syncthreads();                                     // every warp is done with this buffer
-        if (tid == 0 && s + kStages < n_run) issue_stage(s + kStages);
+        if (tid == 0 && s + kStages < n_run) issue_stage(s + kStages);   // n_run <= n_stage
     }
 
     // seed (detectors >= 1): multiply by exp(+2 pi i f_last (tau_I - tau_0)), f_last = frequency of this
@@ -900,6 +904,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             zr[i] = nr; zi[i] = ni;
         }
     }
+    g += (uint32_t)n_issued;                                 // every issued stage has been waited for
     if (MULTI) {                                             // fixed xor tree over the proposal's lanes
         for (int o = lpp >> 1; o > 0; o >>= 1) {
 #pragma unroll
@@ -910,12 +915,14 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
         }
     }
 
-    if (a.n_chunks == 1) {
+    const int n_seg = seg.count;                             // segments of this tile, summed in ascending bin order
+    if (n_seg == 1) {
         if (sub == 0 && live) finish_proposal<NDET, ISCO>(a, b, load_finish_rec<NDET, ISCO>(a, b), zr, zi);
         return;
     }
-    // stage 1 -> workspace: partial[((tile*n_chunks + chunk)*2*NDET + comp)*PT + pic]
-    double *part = a.partial + ((tile * a.n_chunks + chunk) * (int64_t)(2 * NDET)) * PT;
+    // stage 1 -> workspace: partial[(slot*2*NDET + comp)*PT + pic], slot = cta + tile (consecutive along the tile)
+    const int64_t slot0 = seg.first_cta + tile;              // slot of the tile's first segment
+    double *part = a.partial + (seg.slot * (int64_t)(2 * NDET)) * PT;
     if (sub == 0) {
 #pragma unroll
         for (int i = 0; i < NDET; ++i) {
@@ -923,29 +930,28 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             part[(2 * i + 1) * PT + pic] = zi[i];
         }
     }
-    // Ordered sum of `count` entries (chunks or groups) of one proposal: entry e, component q at base[(e*2*NDET+q)*PT].
+    // Ordered sum of `count` entries (segments or groups) of one proposal: entry e, component q at base[(e*2*NDET+q)*PT].
     // Loads of kFinishBatch entries are issued together (the sum is latency-bound on L2 otherwise); the additions
     // stay in index order, so the result does not depend on the batching.
     auto ordered_sum = [&](const double *base, int count, double (&sr)[NDET], double (&si)[NDET]) {
         constexpr int kFinishBatch = 8;
-        int c = 0;
-        for (; c + kFinishBatch <= count; c += kFinishBatch) {
+        for (int c = 0; c < count; c += kFinishBatch) {
+            // the last batch may be short: its loads are clamped to the last entry and its additions masked, so that
+            // a remainder costs one round trip to L2 like a full batch (the finish is a chain of L2 latencies)
             double v[kFinishBatch][2 * NDET];
 #pragma unroll
-            for (int u = 0; u < kFinishBatch; ++u)
+            for (int u = 0; u < kFinishBatch; ++u) {
+                const int e = min(c + u, count - 1);
 #pragma unroll
                 for (int q = 0; q < 2 * NDET; ++q)
-                    v[u][q] = __ldcg(base + ((int64_t)(c + u) * 2 * NDET + q) * PT);
+                    v[u][q] = __ldcg(base + ((int64_t)e * 2 * NDET + q) * PT);
+            }
 #pragma unroll
-            for (int u = 0; u < kFinishBatch; ++u)
+            for (int u = 0; u < kFinishBatch; ++u) {
+                if (c + u < count) {
 #pragma unroll
-                for (int i = 0; i < NDET; ++i) { sr[i] += v[u][2 * i]; si[i] += v[u][2 * i + 1]; }
-        }
-        for (; c < count; ++c) {
-#pragma unroll
-            for (int i = 0; i < NDET; ++i) {
-                sr[i] += __ldcg(base + ((int64_t)c * 2 * NDET + 2 * i) * PT);
-                si[i] += __ldcg(base + ((int64_t)c * 2 * NDET + 2 * i + 1) * PT);
+                    for (int i = 0; i < NDET; ++i) { sr[i] += v[u][2 * i]; si[i] += v[u][2 * i + 1]; }
+                }
             }
         }
     };
@@ -954,14 +960,15 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
     const FinishRec<NDET> frec = load_finish_rec<NDET, ISCO>(a, b_fin < a.n_prop ? b_fin : a.n_prop - 1);
     __threadfence();
     __syncthreads();
-    unsigned int last_ticket = (unsigned)(a.n_chunks - 1);
-    if (a.n_groups > 1) {
-        // Two-level finish for many chunks (a single CTA summing hundreds of chunk partials is bound by one SM's L2
-        // bandwidth): the last CTA of each group of kFinishGroup chunks sums that group in chunk order, and the
-        // last group to finish sums the group sums in group order.  The order is fixed by (n_chunks, kFinishGroup).
-        const int group = chunk / kFinishGroup;
-        const int gsize = min(kFinishGroup, a.n_chunks - group * kFinishGroup);
-        unsigned int *gt = a.gtickets + tile * a.n_groups + group;
+    const int n_groups = n_seg >= kFinishTwoLevelFrom ? (n_seg + kFinishGroup - 1) / kFinishGroup : 1;
+    unsigned int last_ticket = (unsigned)(n_seg - 1);
+    if (n_groups > 1) {
+        // Two-level finish for many segments (a single CTA summing hundreds of partials is bound by one SM's L2
+        // bandwidth): the last CTA of each group of kFinishGroup segments sums that group in order, and the
+        // last group to finish sums the group sums in group order.  The order is fixed by (n_seg, kFinishGroup).
+        const int group = seg.index / kFinishGroup;
+        const int gsize = min(kFinishGroup, n_seg - group * kFinishGroup);
+        unsigned int *gt = a.gtickets + tile * a.gmax + group;
         if (tid == 0) s_ticket = atomicAdd(gt, 1u);
         __syncthreads();
         if (s_ticket != (unsigned)(gsize - 1)) return;
@@ -970,29 +977,28 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             double sr[NDET], si[NDET];
 #pragma unroll
             for (int i = 0; i < NDET; ++i) { sr[i] = 0.0; si[i] = 0.0; }
-            ordered_sum(a.partial + ((tile * a.n_chunks + (int64_t)group * kFinishGroup) * (int64_t)(2 * NDET)) * PT + tid,
-                        gsize, sr, si);
-            double *gp = a.gpartial + ((tile * a.n_groups + group) * (int64_t)(2 * NDET)) * PT + tid;
+            ordered_sum(a.partial + ((slot0 + (int64_t)group * kFinishGroup) * (int64_t)(2 * NDET)) * PT + tid, gsize, sr, si);
+            double *gp = a.gpartial + ((tile * a.gmax + group) * (int64_t)(2 * NDET)) * PT + tid;
 #pragma unroll
             for (int i = 0; i < NDET; ++i) { gp[(2 * i) * PT] = sr[i]; gp[(2 * i + 1) * PT] = si[i]; }
         }
         if (tid == 0) *gt = 0u;
         __threadfence();
         __syncthreads();
-        last_ticket = (unsigned)(a.n_groups - 1);
+        last_ticket = (unsigned)(n_groups - 1);
     }
     if (tid == 0) s_ticket = atomicAdd(&a.tickets[tile], 1u);
     __syncthreads();
     if (s_ticket != last_ticket) return;
-    // stage 2 (last CTA of the tile): chunks (or group sums) added in index order
+    // stage 2 (last CTA of the tile): segments (or group sums) added in index order
     __threadfence();
     {   // Small tiles (multi-lane layouts): all threads pull the tile's partials into the now idle stage buffers in
         // one round trip to L2, and the ordered sums read shared memory.  Same additions in the same order as the
         // direct path below, so the bits do not depend on which path runs.
-        const int nvals = PT * 2 * NDET * a.n_chunks;
-        if (MULTI && a.n_groups == 1 && nvals <= kStages * NP * kStageBins * 2) {
+        const int nvals = PT * 2 * NDET * n_seg;
+        if (MULTI && n_groups == 1 && nvals <= kStages * NP * kStageBins * 2) {
             double *sh = reinterpret_cast<double *>(smem_raw);
-            const double *src = a.partial + (tile * a.n_chunks * (int64_t)(2 * NDET)) * PT;
+            const double *src = a.partial + (slot0 * (int64_t)(2 * NDET)) * PT;
             for (int i = tid; i < nvals; i += kThreads) sh[i] = __ldcg(src + i);
             __syncthreads();
             if (tid < PT) {
@@ -1001,7 +1007,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                     double sr[NDET], si[NDET];
 #pragma unroll
                     for (int i = 0; i < NDET; ++i) { sr[i] = 0.0; si[i] = 0.0; }
-                    for (int c = 0; c < a.n_chunks; ++c) {
+                    for (int c = 0; c < n_seg; ++c) {
 #pragma unroll
                         for (int i = 0; i < NDET; ++i) {
                             sr[i] += sh[(c * 2 * NDET + 2 * i) * PT + tid];
@@ -1012,6 +1018,7 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
                 }
             }
             if (tid == 0) a.tickets[tile] = 0u;
+            __syncthreads();                                 // the stage buffers are free again for the next segment
             return;
         }
     }
@@ -1021,14 +1028,43 @@ __global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedAr
             double sr[NDET], si[NDET];
 #pragma unroll
             for (int i = 0; i < NDET; ++i) { sr[i] = 0.0; si[i] = 0.0; }
-            if (a.n_groups > 1)
-                ordered_sum(a.gpartial + (tile * a.n_groups * (int64_t)(2 * NDET)) * PT + tid, a.n_groups, sr, si);
+            if (n_groups > 1)
+                ordered_sum(a.gpartial + (tile * a.gmax * (int64_t)(2 * NDET)) * PT + tid, n_groups, sr, si);
             else
-                ordered_sum(a.partial + (tile * a.n_chunks * (int64_t)(2 * NDET)) * PT + tid, a.n_chunks, sr, si);
+                ordered_sum(a.partial + (slot0 * (int64_t)(2 * NDET)) * PT + tid, n_seg, sr, si);
             finish_proposal<NDET, ISCO>(a, bb, frec, sr, si);
         }
     }
     if (tid == 0) a.tickets[tile] = 0u;                      // self-reset for the next call
+}
+
+template <int NDET, bool MULTI, bool ISCO, bool TIDAL>
+__global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedArgs a)
+{
+    constexpr int NP = kBasisPlanes + NDET;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + (size_t)kStages * NP * kStageBins * sizeof(double2));
+    __shared__ unsigned int s_ticket;
+    __shared__ int s_relmax;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kStages; ++s) mbar_init(&bars[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    // this CTA's range of the flattened (tile, bin) space, one segment per tile it touches
+    const int64_t cta = blockIdx.x;
+    const int64_t w_end = work_begin(cta + 1, a.work, a.n_cta);
+    uint32_t g = 0;
+    bool first = true;
+    for (int64_t w = work_begin(cta, a.work, a.n_cta); w < w_end;) {
+        const Segment seg = segment_at(w, w_end, cta, a.n_bins, a.work, a.n_cta);
+        fused_segment<NDET, MULTI, ISCO, TIDAL>(a, seg, g, first, smem_raw, s_ticket, s_relmax);
+        w += seg.j1 - seg.j0;
+        first = false;
+        if (w < w_end) __syncthreads();                      // s_ticket / s_relmax / stage buffers change hands
+    }
+    if (first) pdl_wait_primary();                           // an empty range still orders itself after the setup kernel
 }
 
 size_t fused_smem_bytes(int n_det)
@@ -1064,11 +1100,12 @@ cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, cons
 {
     FusedArgs a;
     a.planes = t.planes; a.rec = rec; a.n_pad = t.n_pad; a.n_bins = t.n_bins; a.n_prop = n_prop;
-    a.rec_stride = rec_stride; a.n_chunks = plan.n_chunks; a.lpp = plan.lpp; a.f0 = t.f0; a.delta_f = t.delta_f;
+    a.rec_stride = rec_stride; a.lpp = plan.lpp; a.f0 = t.f0; a.delta_f = t.delta_f;
+    a.work = plan.n_tiles * t.n_bins; a.n_cta = plan.n_cta; a.gmax = plan.gmax;
     for (int i = 0; i < GW_MAX_DET; ++i) a.i7[i] = t.i7[i];
     a.partial = partial; a.tickets = tickets; a.lnl = lnl_out; a.parts = parts_out;
-    a.n_groups = plan.n_groups; a.gpartial = gpartial; a.gtickets = gtickets;
-    const int64_t blocks = plan.n_tiles * plan.n_chunks;
+    a.gpartial = gpartial; a.gtickets = gtickets;
+    const int64_t blocks = plan.n_cta;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     *launches += 1;
     a.i7cum = t.i7cum; a.phase_marginal = t.phase_marginal;
@@ -1121,6 +1158,7 @@ static cudaError_t configure_one()
 cudaError_t configure_kernels(int *out)
 {
     cudaError_t e;
+
     if ((e = configure_one<1>()) != cudaSuccess) return e;
     if ((e = configure_one<2>()) != cudaSuccess) return e;
     if ((e = configure_one<3>()) != cudaSuccess) return e;

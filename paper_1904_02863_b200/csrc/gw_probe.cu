@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(256) store_probe_kernel(double2 *__restrict__ 
 {
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += stride)
-        __stcs(dst + i, make_double2(v, (double)i));
+        __stcs(dst + i, make_double2(v, v));
 }
 
 __global__ void __launch_bounds__(256) load_probe_kernel(const double2 *__restrict__ src, int64_t n16, double *sink)
@@ -164,6 +164,20 @@ cudaError_t probe_bandwidth(int store, int64_t bytes, int n_rep, double *gb_per_
     return cudaGetLastError();
 }
 
+// SM clock actually running: one warp per SM spins for `spin_cycles` of clock64() and reads the nanosecond
+// globaltimer on both sides; MHz = cycles / ns * 1e3, median over the SMs.
+__global__ void clock_probe_kernel(long long spin_cycles, double *mhz)
+{
+    if (threadIdx.x != 0) return;
+    unsigned long long t0, t1;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t0));
+    const long long c0 = clock64();
+    long long c1;
+    do { c1 = clock64(); } while (c1 - c0 < spin_cycles);
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t1));
+    mhz[blockIdx.x] = (double)(c1 - c0) / (double)(t1 - t0) * 1.0e3;
+}
+
 bool arch_ok()
 {
     int dev = 0;
@@ -180,6 +194,28 @@ int gw_probe_fp64_fma_rate(int n_iter, int mode, double *fma_per_s, double *elap
     if (n_iter < 1 || mode < 0 || mode > 5) return -1;
     if (!arch_ok()) return -4;
     return probe_fma_rate(n_iter, mode, fma_per_s, elapsed_ms, (cudaStream_t)cuda_stream) == cudaSuccess ? 0 : -3;
+}
+
+int gw_probe_sm_clock(double *mhz_median, void *cuda_stream)
+{
+    if (!mhz_median) return -1;
+    if (!arch_ok()) return -4;
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    double *d = nullptr;
+    if (cudaMalloc(&d, sizeof(double) * sms) != cudaSuccess) return -3;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    clock_probe_kernel<<<sms, 32, 0, s>>>(60000, d);          // ~30 us at 2 GHz: long against the 32 ns timer tick
+    double h[1024];
+    cudaError_t e = cudaMemcpyAsync(h, d, sizeof(double) * (sms < 1024 ? sms : 1024), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(d);
+    if (e != cudaSuccess) return -3;
+    const int n = sms < 1024 ? sms : 1024;
+    for (int i = 1; i < n; ++i) { const double v = h[i]; int j = i; while (j > 0 && h[j - 1] > v) { h[j] = h[j - 1]; --j; } h[j] = v; }
+    *mhz_median = h[n / 2];
+    return 0;
 }
 
 int gw_probe_store_bandwidth(int64_t bytes, int n_rep, double *gb_per_s, double *best_ms, void *cuda_stream)

@@ -12,7 +12,7 @@ import json
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-EXPORTS = ("gw_probe_fp64_fma_rate", "gw_probe_store_bandwidth", "gw_probe_load_bandwidth")
+EXPORTS = ("gw_probe_fp64_fma_rate", "gw_probe_sm_clock", "gw_probe_store_bandwidth", "gw_probe_load_bandwidth")
 MODES = {0: "fma(v, imm, imm): one register operand", 1: "fma(a, b, v): three distinct register operands",
          2: "fma(a, m, v): three register operands, one shared by consecutive instructions",
          3: "mma.sync m8n8k4 f64 (DMMA)",
@@ -34,6 +34,7 @@ def load_library():
         lib = ctypes.CDLL(path)
         vp, i64, ci, dp = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.POINTER(ctypes.c_double)
         lib.gw_probe_fp64_fma_rate.argtypes = [ci, ci, dp, dp, vp]
+        lib.gw_probe_sm_clock.argtypes = [dp, vp]
         lib.gw_probe_store_bandwidth.argtypes = [i64, ci, dp, dp, vp]
         lib.gw_probe_load_bandwidth.argtypes = [i64, ci, dp, dp, vp]
         for n in EXPORTS:
@@ -55,6 +56,15 @@ def fp64_fma_rate(n_iter: int = 4096, mode: int = 0, stream=None):
     if rc != 0:
         raise RuntimeError(f"gw_probe_fp64_fma_rate: error {rc}")
     return rate.value, ms.value
+
+
+def sm_clock_mhz(stream=None) -> float:
+    """The SM clock actually running (MHz, median over SMs), measured right behind whatever the stream just ran."""
+    mhz = ctypes.c_double()
+    rc = load_library().gw_probe_sm_clock(ctypes.byref(mhz), _stream_ptr(stream))
+    if rc != 0:
+        raise RuntimeError(f"gw_probe_sm_clock: error {rc}")
+    return mhz.value
 
 
 def _bandwidth(fn, n_bytes, n_rep, stream):
@@ -82,6 +92,8 @@ def main():
         best = max(fp64_fma_rate(1 << 13, mode)[0] for _ in range(3))
         out[f"fp64_mode_{mode}"] = {"pattern": what, "fma_per_s": best, "tflops": 2 * best / 1e12}
         print(f"mode {mode}: {best / 1e12:6.2f} T-FMA/s = {2 * best / 1e12:6.2f} TFLOP/s   {what}")
+    out["sm_clock_after_fp64_probe_mhz"] = sm_clock_mhz()
+    print(f"SM clock right after the fp64 probes: {out['sm_clock_after_fp64_probe_mhz']:.0f} MHz")
     for name, fn in (("store", store_bandwidth), ("load", load_bandwidth)):
         gbs, ms = fn()
         out[f"hbm_{name}_GBps"] = gbs
