@@ -24,16 +24,27 @@ _LIB = os.path.join(_HERE, "libgw_oracle.so")
 NPARAM = 11          # Mc, q, chi1, chi2, DL, tc, phic, cos(iota), ra, dec, psi
 DET_ROW = 13         # kind, vertex[3], xarm[3], yarm[3], fplus, fcross, dt
 
+_POP_SRC = os.path.join(_HERE, "gw_pop_oracle.c")
+_POP_LIB = os.path.join(_HERE, "libgw_pop_oracle.so")
+POP_NTHETA = 6       # m1, q, a1, a2, cos tilt1, cos tilt2
+POP_NLAMBDA = 12     # alpha, m_min, m_max, lam, m_pp, sig_pp, beta_q, alpha_chi, beta_chi, xi, sig_1, sig_2
+
 _lib = None
+_pop_lib = None
+
+
+def _compile(src: str, lib: str, force: bool) -> str:
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
+        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+               "-Wall", "-Wextra", "-o", lib, src, "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+    return lib
 
 
 def build(force: bool = False) -> str:
-    """Compile gw_oracle.c with gcc (-O2, no fast-math, OpenMP over proposals)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-               "-Wall", "-Wextra", "-o", _LIB, _SRC, "-lm"]
-        subprocess.run(cmd, check=True, cwd=_HERE)
-    return _LIB
+    """Compile gw_oracle.c and gw_pop_oracle.c with gcc (-O2, no fast-math, OpenMP over proposals / events)."""
+    _compile(_POP_SRC, _POP_LIB, force)
+    return _compile(_SRC, _LIB, force)
 
 
 def _load():
@@ -220,3 +231,72 @@ def lnl_phase_marginal(parts) -> np.ndarray:
     out = np.empty(p.shape[0])
     _load().gwo_lnl_phase_marginal(p.shape[0], p.shape[1], _p(p), _p(out))
     return out
+
+
+# ---- population likelihood, Eq. 3 (gw_pop_oracle.c) ------------------------------------------------------
+def _pop():
+    global _pop_lib
+    if _pop_lib is None:
+        build()
+        lib = ctypes.CDLL(_POP_LIB)
+        dp, i64, cint, dbl = ctypes.POINTER(ctypes.c_double), ctypes.c_int64, ctypes.c_int, ctypes.c_double
+        for name, args in (("gwpo_powerlaw_pdf", [dbl] * 4), ("gwpo_truncnorm_pdf", [dbl] * 5),
+                           ("gwpo_mass_pdf", [dbl, dp]), ("gwpo_ratio_pdf", [dbl, dbl, dp]),
+                           ("gwpo_beta_pdf", [dbl] * 3), ("gwpo_tilt_pdf", [dbl, dbl, dp]),
+                           ("gwpo_population_pdf", [dp, dp])):
+            f = getattr(lib, name)
+            f.argtypes, f.restype = args, dbl
+        lib.gwpo_lambda_valid.argtypes, lib.gwpo_lambda_valid.restype = [dp], cint
+        lib.gwpo_lnl.argtypes = [i64, i64, dp, dp, i64, dp, cint, dp, dp]
+        lib.gwpo_lnl.restype = cint
+        _pop_lib = lib
+    return _pop_lib
+
+
+def pop_powerlaw_pdf(x, alpha, lo, hi) -> float:
+    return _pop().gwpo_powerlaw_pdf(float(x), float(alpha), float(lo), float(hi))
+
+
+def pop_truncnorm_pdf(x, mu, sigma, lo, hi) -> float:
+    return _pop().gwpo_truncnorm_pdf(float(x), float(mu), float(sigma), float(lo), float(hi))
+
+
+def pop_mass_pdf(m1, lam) -> float:
+    return _pop().gwpo_mass_pdf(float(m1), _p(_f64(lam, (POP_NLAMBDA,))))
+
+
+def pop_ratio_pdf(q, m1, lam) -> float:
+    return _pop().gwpo_ratio_pdf(float(q), float(m1), _p(_f64(lam, (POP_NLAMBDA,))))
+
+
+def pop_beta_pdf(a, alpha_chi, beta_chi) -> float:
+    return _pop().gwpo_beta_pdf(float(a), float(alpha_chi), float(beta_chi))
+
+
+def pop_tilt_pdf(c1, c2, lam) -> float:
+    return _pop().gwpo_tilt_pdf(float(c1), float(c2), _p(_f64(lam, (POP_NLAMBDA,))))
+
+
+def pop_pdf(theta, lam) -> float:
+    """p(theta | Lambda) for one theta[6] and one Lambda[12]."""
+    return _pop().gwpo_population_pdf(_p(_f64(theta, (POP_NTHETA,))), _p(_f64(lam, (POP_NLAMBDA,))))
+
+
+def pop_lambda_valid(lam) -> bool:
+    return bool(_pop().gwpo_lambda_valid(_p(_f64(lam, (POP_NLAMBDA,)))))
+
+
+def pop_lnl(samples, prior, lambdas, n_threads=0):
+    """Eq. 3 without its prefactor -> (lnL[B], inner sums [B][N], threads used).
+    samples [N][n][6], prior [N][n], lambdas [B][12]."""
+    s = _f64(samples)
+    n_events, n_samples = s.shape[0], s.shape[1]
+    s = s.reshape(n_events, n_samples, POP_NTHETA)
+    p0 = _f64(prior, (n_events, n_samples))
+    lam = _f64(lambdas).reshape(-1, POP_NLAMBDA)
+    out = np.empty(lam.shape[0])
+    inner = np.empty((lam.shape[0], n_events))
+    used = _pop().gwpo_lnl(n_events, n_samples, _p(s), _p(p0), lam.shape[0], _p(lam), int(n_threads), _p(out), _p(inner))
+    if used < 0:
+        raise MemoryError("gwpo_lnl")
+    return out, inner, used

@@ -206,3 +206,67 @@ def make_data(cfg: Config, waveform_fn: WaveformFn) -> np.ndarray:
     th = np.asarray(cfg.theta_inj, dtype=np.float64)[None, :]
     s = np.asarray(waveform_fn(frequency_grid(cfg), detectors(cfg), cfg.gmst, th, cfg.spin_order))
     return s.reshape(cfg.n_det, cfg.n_bins) + noise(cfg)
+
+
+# ---- population likelihood workloads (section IV, Eq. 3) --------------------------
+# Synthetic posterior samples stand in for the GWTC-1 release the paper used (ten events, >= 2e4 samples
+# each) and for its projected catalogues (up to ~4e6 samples); nothing here evaluates a population model.
+POP_NTHETA = 6       # m1 [Msun], q, a1, a2, cos tilt1, cos tilt2
+POP_NLAMBDA = 12     # alpha, m_min, m_max, lam, m_pp, sig_pp, beta_q, alpha_chi, beta_chi, xi, sig_1, sig_2
+POP_M1_RANGE = (2.5, 95.0)
+
+
+@dataclass(frozen=True)
+class PopConfig:
+    name: str
+    index: int
+    n_events: int
+    n_samples: int
+    batch: int           # hyper-parameter proposals Lambda per call
+
+    @property
+    def seed_samples(self) -> int:
+        return BASE_SEED + 100 + 10 * self.index + 1
+
+    @property
+    def seed_prop(self) -> int:
+        return BASE_SEED + 100 + 10 * self.index + 2
+
+
+POP_CONFIGS = {
+    "P0": PopConfig("P0", 0, 10, 2000, 64),        # small: the oracle finishes in seconds
+    "P1": PopConfig("P1", 1, 10, 20000, 64),       # 2e5 samples: the size of the GWTC-1 release
+    "P2": PopConfig("P2", 2, 100, 40000, 64),      # 4e6 samples: where the paper's P100 saturates
+}
+
+
+def pop_samples(cfg: PopConfig) -> Tuple[np.ndarray, np.ndarray]:
+    """(samples [N][n][6], prior [N][n]): per event a Gaussian cloud around a random centre, folded into the domain;
+    the prior the clouds are weighted by is p(theta | 0) = (2 m1 / (hi^2 - lo^2)) * 1 * 1 * 1 * (1/4) -- flat in the
+    component masses, in both spin magnitudes and in both tilt cosines."""
+    rng = np.random.Generator(np.random.PCG64(cfg.seed_samples))
+    N, n = cfg.n_events, cfg.n_samples
+    lo = np.array([POP_M1_RANGE[0], 0.05, 0.005, 0.005, -0.999, -0.999])
+    hi = np.array([POP_M1_RANGE[1], 1.0, 0.995, 0.995, 0.999, 0.999])
+    c_lo = np.array([8.0, 0.5, 0.05, 0.05, -0.5, -0.5])
+    c_hi = np.array([45.0, 0.95, 0.6, 0.6, 0.9, 0.9])
+    centre = c_lo + (c_hi - c_lo) * rng.random((N, POP_NTHETA))
+    width = np.array([0.0, 0.12, 0.15, 0.15, 0.35, 0.35]) + np.zeros((N, POP_NTHETA))
+    width[:, 0] = 0.1 * centre[:, 0]
+    x = centre[:, None, :] + width[:, None, :] * rng.standard_normal((N, n, POP_NTHETA))
+    span = hi - lo                                      # fold into [lo, hi] by reflection
+    y = np.mod(x - lo, 2.0 * span)
+    x = lo + np.where(y > span, 2.0 * span - y, y)
+    prior = 2.0 * x[..., 0] / (POP_M1_RANGE[1] ** 2 - POP_M1_RANGE[0] ** 2) * 0.25
+    return np.ascontiguousarray(x), np.ascontiguousarray(prior)
+
+
+def pop_lambdas(cfg: PopConfig, batch: Optional[int] = None) -> np.ndarray:
+    """Lambda[B][12] drawn uniformly from the usual prior ranges of a population analysis; row 0 is a fixed, typical
+    point.  (beta_q stays away from -1 and alpha from 1, the two removable singularities of the normalisations.)"""
+    rng = np.random.Generator(np.random.PCG64(cfg.seed_prop))
+    lo = np.array([1.2, 3.0, 50.0, 0.0, 25.0, 1.0, -0.5, 1.0, 1.0, 0.0, 0.3, 0.3])
+    hi = np.array([4.0, 8.0, 90.0, 0.3, 40.0, 8.0, 4.0, 5.0, 6.0, 1.0, 3.0, 3.0])
+    lam = lo + (hi - lo) * rng.random((cfg.batch, POP_NLAMBDA))
+    lam[0] = (2.35, 5.0, 70.0, 0.1, 33.0, 5.0, 1.3, 2.0, 4.0, 0.6, 1.0, 1.5)
+    return np.ascontiguousarray(lam if batch is None else lam[:batch])
