@@ -1,7 +1,7 @@
 #!/usr/bin/env python3
 """Build the CUDA libraries with nvcc for sm_100a, in-tree:
 
-    csrc/libgwlnl.so    the product library: C-ABI of include/gwlnl.h, include/gwlnl_tuning.h
+    csrc/libgwlnl.so    the product library: C-ABI of include/gwlnl.h, include/gwlnl_tuning.h, include/gwpop.h
     csrc/libgwprobe.so  measurement aids only (include/gwprobe.h): fp64-rate and HBM store / load bandwidth probes
 
     python paper_1904_02863_b200/csrc/build.py [--force] [--verbose]
@@ -15,8 +15,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
 INC = os.path.join(ROOT, "include")
-SOURCES = ["gw_api.cu", "gw_kernels.cu"]
-HEADERS = ["gw_internal.h", "gw_math.cuh", os.path.join(INC, "gwlnl.h"), os.path.join(INC, "gwlnl_tuning.h")]
+SOURCES = ["gw_api.cu", "gw_kernels.cu", "gw_pop.cu"]
+HEADERS = ["gw_internal.h", "gw_math.cuh", os.path.join(INC, "gwlnl.h"), os.path.join(INC, "gwlnl_tuning.h"),
+           os.path.join(INC, "gwpop.h")]
 LIB = os.path.join(HERE, "libgwlnl.so")
 PROBE_SOURCES = ["gw_probe.cu"]
 PROBE_HEADERS = [os.path.join(INC, "gwprobe.h")]

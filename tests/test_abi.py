@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-COVERED_HEADERS = ("gwlnl.h", "gwlnl_tuning.h", "gwprobe.h")
+COVERED_HEADERS = ("gwlnl.h", "gwlnl_tuning.h", "gwpop.h", "gwprobe.h")
 
 
 @pytest.fixture(scope="module")
@@ -36,6 +36,11 @@ def test_header_symbols_are_exported(lib):
     assert sorted(binding.TUNING_EXPORTS) == tuning and tuning
     for n in tuning:
         assert hasattr(lib, n), f"{n} declared in gwlnl_tuning.h but not exported"
+    from paper_1904_02863_b200 import population
+    pop = _declared_functions("gwpop.h")
+    assert sorted(population.EXPORTS) == pop and {"gw_pop_ctx_create", "gw_pop_lnl_batch", "gw_pop_ctx_destroy"} <= set(pop)
+    for n in pop:
+        assert hasattr(lib, n), f"{n} declared in gwpop.h but not exported"
     # the probes (fp64 rate, HBM bandwidth) live in their own library, not in the product library
     assert not any(hasattr(lib, n) for n in _declared_functions("gwprobe.h"))
 
@@ -66,6 +71,15 @@ def test_no_compute_calls(lib):
     assert lib.gw_waveform_batch(None, 1, None, None, None) == -1
     assert lib.gw_ctx_reserve(None, 8) == -1
     assert lib.gw_last_cuda_error(None) == 0 and lib.gw_ctx_launch_count(None) == 0
+    from paper_1904_02863_b200 import population
+    population._lib()
+    assert lib.gw_pop_ctx_destroy(None) == 0 and lib.gw_pop_ctx_launch_count(None) == 0
+    assert lib.gw_pop_ctx_info(None, None, None, None, None) == -1
+    assert lib.gw_pop_lnl_batch(None, 1, None, None, None) == -1
+    h = ctypes.c_void_p()
+    x = np.zeros(12)
+    assert lib.gw_pop_ctx_create(ctypes.byref(h), 0, 2, x.ctypes.data, x.ctypes.data, 1, None) == -1 and not h
+    assert lib.gw_pop_ctx_create(ctypes.byref(h), 1, 2, None, x.ctypes.data, 1, None) == -1 and not h
 
 
 def test_create_rejects_bad_arguments_before_touching_cuda(lib):
