@@ -198,6 +198,125 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_population(args):
+    """--workload P0|P1|P2[:B]: the population likelihood, Eq. 3.  A step is one
+    gw_pop_lnl_batch call: B hyper-parameter proposals over the N x n resident samples.  HBM-bound map-reduce: the
+    roofline is read against bytes (7 input arrays of the paper's data flow, PAPER.md:109, = 56 B per sample and pass;
+    the kernel streams 8 transformed planes = 64 B)."""
+    import torch
+    from paper_1904_02863_b200.csrc import build as csrc_build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        raise SystemExit("bench.py: the population workload is timed on one GPU")
+    torch.cuda.set_device(0)
+    if os.path.exists(csrc_build.NVCC):
+        csrc_build.build()
+        csrc_build.build_probe()
+    from paper_1904_02863_b200 import inputs, probes
+    from paper_1904_02863_b200.population import GwPopContext
+    name, _, b = args.workload.partition(":")
+    cfg = inputs.POP_CONFIGS[name]
+    B = int(b) if b else 1
+    s, p0 = inputs.pop_samples(cfg)
+    lam_all = inputs.pop_lambdas(inputs.PopConfig(cfg.name, cfg.index, cfg.n_events, cfg.n_samples, max(B, cfg.batch)))
+    lam = np.ascontiguousarray(lam_all[:B])
+    ctx = GwPopContext(s, p0, max_batch=B)
+    lam_d = torch.from_numpy(lam).cuda()
+    out = torch.empty(B, dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+    n_samp = cfg.n_events * cfg.n_samples
+    in_l2 = n_samp * 64 <= (100 << 20)
+
+    def step():
+        ctx.lnl_batch(lam_d, out=out)
+
+    probes.fp64_fma_rate(1 << 14)
+    for _ in range(max(3, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    launches0 = ctx.launch_count()
+    with ClockSampler(0) as clk:
+        for i in range(args.steps):
+            flush.fill_(i & 0xff)
+            ev0[i].record(stream); step(); ev1[i].record(stream)
+        clock_after_mhz = probes.sm_clock_mhz()
+        torch.cuda.synchronize()
+    launches = ctx.launch_count() - launches0
+    step_ms = np.array([a.elapsed_time(b_) for a, b_ in zip(ev0, ev1)])
+    value = B * args.steps / (step_ms.sum() * 1e-3)
+    ctx.kernel_timing(True)
+    k_ms = []
+    for i in range(args.steps):
+        flush.fill_(i & 0xff)
+        step()
+        k_ms.append(ctx.last_kernel_ms())
+    ctx.kernel_timing(False)
+    k_ms = np.array(k_ms)
+    main_ms = float(k_ms[:, 1].mean())
+    passes = 1 if B <= 2 else (B + 3) // 4
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    load_gbs, _ = probes.load_bandwidth(2 << 30, 10)
+    alg_bytes = 56.0 * n_samp * passes
+    achieved = alg_bytes / (main_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "pop_main_kernel<%d>" % (B if B <= 2 else 4), "achieved": achieved, "peak": hbm,
+                "unit": "GB/s", "frac": achieved / hbm, "traffic": None,
+                "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)",
+                "pure_load_ceiling_GBps": load_gbs, "frac_of_pure_load": achieved / load_gbs,
+                "algorithmic_bytes_per_launch": alg_bytes, "bytes_streamed_per_launch": 64.0 * n_samp * passes,
+                "passes_over_the_samples": passes, "proposals_per_pass": min(B, 4),
+                "sample_lambda_pairs_per_s": n_samp * B / (main_ms * 1e-3),
+                "kernel_ms": main_ms, "kernel_ms_median": float(np.median(k_ms[:, 1])), "kernel_ms_best": float(k_ms[:, 1].min()),
+                "setup_kernel_ms": float(k_ms[:, 0].mean()), "finish_kernel_ms": float(k_ms[:, 2].mean()),
+                "note": "one proposal per pass is HBM-bound; with 4 proposals per pass every plane value read is used four "
+                        "times and the exponentials (4 per sample and proposal) bound the kernel instead"}
+    # end to end: host Lambda in, host lnL out, synchronised
+    lam_pin = torch.from_numpy(lam).pin_memory().numpy()
+    out_pin = torch.empty(B, dtype=torch.float64).pin_memory().numpy()
+    for _ in range(3):
+        ctx.lnl_batch_host(lam_pin, out=out_pin)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ctx.lnl_batch_host(lam_pin, out=out_pin)
+    e2e_s = time.perf_counter() - t0
+    e2e = {"value": B * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(lam.nbytes), "d2h_bytes_per_step": 8 * B,
+           "ms_per_step": 1e3 * e2e_s / args.steps, "api": "gw_pop_lnl_batch_host (host Lambda in, host lnL out, stream synchronised)"}
+    cpu = None
+    if not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        nl = 1
+        t0 = time.perf_counter()
+        _, _, used = oracle.pop_lnl(s, p0, lam_all[:nl], n_threads=os.cpu_count() or 1)
+        dt = time.perf_counter() - t0
+        nl = int(max(1, min(cfg.batch, args.cpu_seconds / max(dt, 1e-3))))
+        t0 = time.perf_counter()
+        _, _, used = oracle.pop_lnl(s, p0, lam_all[:nl], n_threads=os.cpu_count() or 1)
+        dt = time.perf_counter() - t0
+        cpu = {"value": nl / dt, "unit": UNIT, "cores": used, "kind": "oracle",
+               "sample": f"{nl} hyper-parameter proposals over all {cfg.n_events} x {cfg.n_samples} samples, {dt:.1f} s wall"}
+    clocks = clk.summary()
+    clocks["sm_mhz_measured_after_timed_region"] = clock_after_mhz
+    ctx.close()
+    line = {"metric": "population likelihood evals/sec (fp64, PAPER.md Eq. 3)", "value": value, "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": float(step_ms.mean()),
+            "ms_per_step_median": float(np.median(step_ms)), "ms_per_step_best": float(step_ms.min()),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{name}: {cfg.n_events} events x {cfg.n_samples} samples, {B} hyper-parameter proposals per call",
+                       "samples": n_samp, "global_batch": B,
+                       "l2": "flushed before every timed step (256 MiB write)" + ("; the sample planes (%d MB) would otherwise stay in L2" % (n_samp * 64 >> 20) if in_l2 else "; the sample planes exceed L2")},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line))
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -451,7 +570,11 @@ def main():
     ap.add_argument("--tidal-order", type=int, default=0, choices=[0, 1, 2],
                     help="NEXT-1 option: 5PN (1) or 5PN + 6PN (2) tidal phase terms; theta rows of 13 columns")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.workload.startswith("P"):
+        if args.impl == "reference":
+            raise SystemExit("bench.py: --impl reference covers the single-event workloads C0..C4")
+        run_population(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

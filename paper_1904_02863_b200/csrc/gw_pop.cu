@@ -17,7 +17,8 @@
 //   T  = (1 - xi)/4 + xi C_1 C_2 exp(-d_1 / (2 sig_1^2) - d_2 / (2 sig_2^2))          tilts
 //   w  = A T / Qn  inside the support (m_min < m1 <= m_max, lq >= ln m_min - lm), else 0
 //   r1 = ln[(1 - lam) C_pl |1 + beta_q| / B(alpha_chi, beta_chi)^2],  r2 = ln[lam C_g |1 + beta_q| / B^2].
-// Four exponentials and one division per (sample, Lambda); 64 bytes of planes per sample and pass.
+// Four exponentials and one division per (sample, Lambda); 64 bytes of planes per sample and pass.  (A hand-written exp --
+// conversion-pipe range reduction, degree-11 Horner -- measured 15 % SLOWER than libdevice's exp here: DESIGN.md section 13.)
 #include <cmath>
 #include <cstring>
 #include <new>
