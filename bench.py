@@ -268,7 +268,8 @@ def run_population(args):
     alg_bytes = 56.0 * n_samp * passes
     achieved = alg_bytes / (main_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "pop_main_kernel<%d>" % (B if B <= 2 else 4), "achieved": achieved, "peak": hbm,
-                "unit": "GB/s", "frac": achieved / hbm, "traffic": None,
+                "unit": "GB/s", "frac": achieved / hbm, "traffic": ncu_traffic("%s:%d" % (name, B))[0],
+                "traffic_source": ncu_traffic("%s:%d" % (name, B))[1],
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)",
                 "pure_load_ceiling_GBps": load_gbs, "frac_of_pure_load": achieved / load_gbs,
                 "algorithmic_bytes_per_launch": alg_bytes, "bytes_streamed_per_launch": 64.0 * n_samp * passes,
@@ -413,6 +414,16 @@ def run_ours(args):
         k_ms.append(b)
     ctx.kernel_timing(False)
     fused_ms = float(np.mean(k_ms))
+    # what the kernel-alone measurement includes besides the kernel: an empty kernel of the same launch shape, timed the same way
+    floor_ms = probes.launch_floor_ms(plan["n_ctas"], 256, 63000, 50)
+    # the sustained rate of a sampler loop: calls back to back between ONE pair of events, no L2 flush, no events inside
+    n_b2b = 50
+    b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    step(); b0.record(stream)
+    for _ in range(n_b2b):
+        step()
+    b1.record(stream); torch.cuda.synchronize()
+    b2b_ms = b0.elapsed_time(b1) / n_b2b
     walg = walg_per_bin(n_det, args.tidal_order)
     wexe = executed_per_bin(n_det, args.tidal_order)
     pairs = float(B) * M                                   # (proposal, bin) pairs with algorithmic work
@@ -439,6 +450,12 @@ def run_ours(args):
                              "fp64 instructions the kernel issues and is the fraction of raw fp64-pipe issue slots",
                 "executed_fp64_per_prop_bin": wexe, "frac_executed": achieved / peak * wexe / walg,
                 "kernel_ms_median": float(np.median(k_ms)), "kernel_ms_best": float(np.min(k_ms)),
+                "launch_floor_ms": floor_ms, "frac_net_of_launch_floor": flops_per_launch / ((fused_ms - floor_ms) * 1e-3) / 1e12 / peak,
+                "launch_floor_note": "kernel_ms is one launch between two CUDA events; an EMPTY kernel of the same launch shape timed "
+                                     "the same way reads launch_floor_ms (gw_probe_launch_floor).  frac uses kernel_ms as measured.",
+                "back_to_back_ms_per_call": b2b_ms, "back_to_back_note": "%d gw_lnl_batch calls (setup + fused kernel, overlapped by "
+                "programmatic dependent launch) between one pair of events, no L2 flush: the sustained rate of a sampler loop" % n_b2b,
+                "frac_back_to_back_step": flops_per_launch / (b2b_ms * 1e-3) / 1e12 / peak,
                 "peak_source": "derived: %d SMs x %d fp64 FMA lanes x 2 flop x %.0f MHz (%s)"
                                % (n_sm, FP64_LANES_PER_SM, sm_max,
                                   "MEASURED_PEAKS.json sm_max_mhz" if "sm_max_mhz" in peaks else "fallback clock, B200_PROFILING.md"),

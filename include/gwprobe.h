@@ -31,6 +31,11 @@ int gw_probe_fp64_fma_rate(int n_iter, int mode, double *fma_per_s, double *elap
  * scale).                                                                                                    */
 int gw_probe_sm_clock(double *mhz_median, void *cuda_stream);
 
+/* The floor of "one kernel timed alone between two CUDA events": median over n_rep of the event-to-event time of an
+ * EMPTY kernel launched with the given grid, block and dynamic shared memory right behind other work on the stream.
+ * On B200 this reads ~6 us whatever the launch shape; bench.py reports it beside every kernel-level time.      */
+int gw_probe_launch_floor(int grid, int block, int dyn_smem_bytes, int n_rep, double *median_ms, void *cuda_stream);
+
 /* Pure-store HBM bandwidth: `bytes` (far larger than the 126 MB L2) written once per pass with 16-byte streaming
  * stores by a grid of 8 CTAs per SM; best of `n_rep` passes after one warm-up pass.  GB/s = bytes / best time.   */
 int gw_probe_store_bandwidth(int64_t bytes, int n_rep, double *gb_per_s, double *best_ms, void *cuda_stream);

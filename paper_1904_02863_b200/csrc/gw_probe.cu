@@ -178,6 +178,10 @@ __global__ void clock_probe_kernel(long long spin_cycles, double *mhz)
     mhz[blockIdx.x] = (double)(c1 - c0) / (double)(t1 - t0) * 1.0e3;
 }
 
+// Event-to-event time of a kernel that does nothing: the floor that any "kernel timed alone between two events"
+// measurement includes (launch latency after the preceding work has drained + completion + the two event records).
+__global__ void empty_probe_kernel(int *p) { if (p && threadIdx.x == 0xffff) *p = 1; }
+
 bool arch_ok()
 {
     int dev = 0;
@@ -215,6 +219,34 @@ int gw_probe_sm_clock(double *mhz_median, void *cuda_stream)
     const int n = sms < 1024 ? sms : 1024;
     for (int i = 1; i < n; ++i) { const double v = h[i]; int j = i; while (j > 0 && h[j - 1] > v) { h[j] = h[j - 1]; --j; } h[j] = v; }
     *mhz_median = h[n / 2];
+    return 0;
+}
+
+int gw_probe_launch_floor(int grid, int block, int dyn_smem_bytes, int n_rep, double *median_ms, void *cuda_stream)
+{
+    if (grid < 1 || block < 1 || block > 1024 || dyn_smem_bytes < 0 || dyn_smem_bytes > 227 * 1024 || n_rep < 1 || n_rep > 4096 || !median_ms)
+        return -1;
+    if (!arch_ok()) return -4;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (cudaFuncSetAttribute(empty_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_smem_bytes) != cudaSuccess) return -3;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    float t[4096];
+    cudaError_t e = cudaSuccess;
+    for (int r = 0; r < n_rep + 3 && e == cudaSuccess; ++r) {          // three warm-up launches
+        empty_probe_kernel<<<148, 128, 0, s>>>(nullptr);              // preceding work on the stream, as in a real step
+        cudaEventRecord(e0, s);
+        empty_probe_kernel<<<grid, block, dyn_smem_bytes, s>>>(nullptr);
+        cudaEventRecord(e1, s);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (r >= 3) t[r - 3] = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (e != cudaSuccess) return -3;
+    for (int i = 1; i < n_rep; ++i) { const float v = t[i]; int j = i; while (j > 0 && t[j - 1] > v) { t[j] = t[j - 1]; --j; } t[j] = v; }
+    *median_ms = t[n_rep / 2];
     return 0;
 }
 

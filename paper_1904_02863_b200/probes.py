@@ -12,7 +12,8 @@ import json
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-EXPORTS = ("gw_probe_fp64_fma_rate", "gw_probe_sm_clock", "gw_probe_store_bandwidth", "gw_probe_load_bandwidth")
+EXPORTS = ("gw_probe_fp64_fma_rate", "gw_probe_sm_clock", "gw_probe_launch_floor", "gw_probe_store_bandwidth",
+           "gw_probe_load_bandwidth")
 MODES = {0: "fma(v, imm, imm): one register operand", 1: "fma(a, b, v): three distinct register operands",
          2: "fma(a, m, v): three register operands, one shared by consecutive instructions",
          3: "mma.sync m8n8k4 f64 (DMMA)",
@@ -35,6 +36,7 @@ def load_library():
         vp, i64, ci, dp = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.POINTER(ctypes.c_double)
         lib.gw_probe_fp64_fma_rate.argtypes = [ci, ci, dp, dp, vp]
         lib.gw_probe_sm_clock.argtypes = [dp, vp]
+        lib.gw_probe_launch_floor.argtypes = [ci, ci, ci, ci, dp, vp]
         lib.gw_probe_store_bandwidth.argtypes = [i64, ci, dp, dp, vp]
         lib.gw_probe_load_bandwidth.argtypes = [i64, ci, dp, dp, vp]
         for n in EXPORTS:
@@ -67,6 +69,16 @@ def sm_clock_mhz(stream=None) -> float:
     return mhz.value
 
 
+def launch_floor_ms(grid: int = 148, block: int = 256, dyn_smem_bytes: int = 0, n_rep: int = 50, stream=None) -> float:
+    """Median event-to-event time (ms) of an empty kernel with this launch shape: what a kernel-alone timing includes."""
+    ms = ctypes.c_double()
+    rc = load_library().gw_probe_launch_floor(int(grid), int(block), int(dyn_smem_bytes), int(n_rep), ctypes.byref(ms),
+                                              _stream_ptr(stream))
+    if rc != 0:
+        raise RuntimeError(f"gw_probe_launch_floor: error {rc}")
+    return ms.value
+
+
 def _bandwidth(fn, n_bytes, n_rep, stream):
     gbs, ms = ctypes.c_double(), ctypes.c_double()
     rc = fn(int(n_bytes), int(n_rep), ctypes.byref(gbs), ctypes.byref(ms), _stream_ptr(stream))
@@ -94,6 +106,8 @@ def main():
         print(f"mode {mode}: {best / 1e12:6.2f} T-FMA/s = {2 * best / 1e12:6.2f} TFLOP/s   {what}")
     out["sm_clock_after_fp64_probe_mhz"] = sm_clock_mhz()
     print(f"SM clock right after the fp64 probes: {out['sm_clock_after_fp64_probe_mhz']:.0f} MHz")
+    out["launch_floor_us"] = 1e3 * launch_floor_ms()
+    print(f"empty kernel between two events: {out['launch_floor_us']:.2f} us")
     for name, fn in (("store", store_bandwidth), ("load", load_bandwidth)):
         gbs, ms = fn()
         out[f"hbm_{name}_GBps"] = gbs
