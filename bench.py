@@ -353,6 +353,10 @@ def run_ours(args):
                     tidal_order=int(args.tidal_order))
     if args.force_grid or args.force_lpp:                 # tuning aid (include/gwlnl_tuning.h): pin the launch shape
         ctx.force_grid(args.force_lpp, args.force_grid)
+    if args.no_cluster:
+        ctx.cluster_finish(False)
+    if args.no_host_graph:
+        ctx.host_graph(False)
     thd = torch.from_numpy(th).cuda()
     lnl = torch.empty(B, dtype=torch.float64, device="cuda")
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
@@ -558,7 +562,7 @@ def run_ours(args):
                 "config": {"workload": f"{name}: {n_det} det x {M} bins x {B} proposals per GPU",
                            "global_batch": B * world, "bins": M, "detectors": n_det, "parallelism": f"proposals sharded x{world}",
                            "l2": "flushed before every timed step: 256 MiB write, then a 256 MiB read of a second buffer (no dirty lines left)", "plan": plan,
-                           "pinned": {"grid": args.force_grid, "lanes_per_prop": args.force_lpp},
+                           "pinned": {"grid": args.force_grid, "lanes_per_prop": args.force_lpp, "no_cluster": bool(args.no_cluster)},
                            "options": {"isco_cut": int(args.isco_cut), "phase_marginal": int(args.phase_marginal),
                                        "tidal_order": int(args.tidal_order)}},
                 "bin_det_proposals_per_s": value * M * n_det,
@@ -582,6 +586,8 @@ def main():
     ap.add_argument("--no-waveform", action="store_true")
     ap.add_argument("--force-grid", type=int, default=0, help="tuning aid: pin the fused kernel's grid to this many CTAs")
     ap.add_argument("--force-lpp", type=int, default=0, help="tuning aid: pin the lanes per proposal (1, 2, ..., 32)")
+    ap.add_argument("--no-host-graph", action="store_true", help="tuning aid: small host calls launch by launch, not through the library's graph")
+    ap.add_argument("--no-cluster", action="store_true", help="tuning aid: small grids through the ticket finish, not clusters")
     ap.add_argument("--isco-cut", action="store_true", help="NEXT-1 option: h = 0 above f_ISCO (not the headline config)")
     ap.add_argument("--phase-marginal", action="store_true", help="NEXT-1 option: lnL marginalised over phi_c")
     ap.add_argument("--tidal-order", type=int, default=0, choices=[0, 1, 2],

@@ -22,6 +22,15 @@ int gw_ctx_force_plan(gw_ctx *ctx, int lanes_per_prop, int n_chunks);
  * whatever the tile count (n_ctas >= 1; 0 leaves the choice to the planner; overrides a pinned n_chunks).       */
 int gw_ctx_force_grid(gw_ctx *ctx, int lanes_per_prop, int64_t n_ctas);
 
+/* Testing / tuning aid: multi-lane grids of 2..16 chunks per tile launch every tile as one thread-block cluster and add
+ * the chunk sums through distributed shared memory (default, enable = 1); 0 sends them through the global partial sums
+ * and the per-tile ticket like every other grid.  Both paths add the same numbers in the same order (identical bits).  */
+int gw_ctx_cluster_finish(gw_ctx *ctx, int enable);
+
+/* Testing / tuning aid: gw_lnl_batch_host sends batches of up to 512 proposals through a library-owned CUDA graph (one
+ * launch per call; default, enable = 1); 0 makes it enqueue the copy and the two kernels one by one like larger batches. */
+int gw_ctx_host_graph(gw_ctx *ctx, int enable);
+
 /* Host-only (no CUDA call): the segments that CTA `cta` of a grid of n_ctas CTAs sweeps when n_tiles proposal tiles
  * of n_bins bins are shared equally -- the same arithmetic the fused kernel runs (csrc/gw_internal.h, segment_at).
  * Writes up to max_rows rows of 6 values (tile, j0, j1, index of the segment within its tile, segments of that tile,

@@ -27,7 +27,7 @@ EXPORTS = (
     "gw_ctx_launch_count", "gw_strerror", "gw_last_cuda_error", "gw_abi_version",
 )
 # include/gwlnl_tuning.h: testing / tuning aids exported by the same library, outside the product boundary
-TUNING_EXPORTS = ("gw_ctx_force_plan", "gw_ctx_force_grid", "gw_plan_cta_segments", "gw_ctx_kernel_timing",
+TUNING_EXPORTS = ("gw_ctx_force_plan", "gw_ctx_force_grid", "gw_ctx_cluster_finish", "gw_ctx_host_graph", "gw_plan_cta_segments", "gw_ctx_kernel_timing",
                   "gw_ctx_last_kernel_ms")
 
 
@@ -84,6 +84,8 @@ def load_library():
     lib.gw_ctx_launch_count.restype = i64
     lib.gw_ctx_force_plan.argtypes = [vp, ci, ci]
     lib.gw_ctx_force_grid.argtypes = [vp, ci, i64]
+    lib.gw_ctx_cluster_finish.argtypes = [vp, ci]
+    lib.gw_ctx_host_graph.argtypes = [vp, ci]
     lib.gw_plan_cta_segments.argtypes = [i64, i64, i64, i64, ci, P(i64)]
     lib.gw_ctx_kernel_timing.argtypes = [vp, ci]
     lib.gw_ctx_last_kernel_ms.argtypes = [vp, P(dbl), P(dbl)]
@@ -226,6 +228,14 @@ class GwContext:
     def force_grid(self, lanes_per_prop: int = 0, n_ctas: int = 0):
         """Pin the grid of lnl_batch: n_ctas CTAs share the (tile, bin) space equally (0 = planner's choice)."""
         _check(self._lib.gw_ctx_force_grid(self._h, int(lanes_per_prop), int(n_ctas)), "gw_ctx_force_grid", self._h)
+
+    def cluster_finish(self, enable: bool):
+        """Tuning aid: cluster / distributed-shared-memory finish of small multi-lane grids on (default) or off."""
+        _check(self._lib.gw_ctx_cluster_finish(self._h, int(bool(enable))), "gw_ctx_cluster_finish", self._h)
+
+    def host_graph(self, enable: bool):
+        """Tuning aid: small lnl_batch_host calls through the library-owned CUDA graph (default) or launch by launch."""
+        _check(self._lib.gw_ctx_host_graph(self._h, int(bool(enable))), "gw_ctx_host_graph", self._h)
 
     def kernel_timing(self, enable: bool):
         _check(self._lib.gw_ctx_kernel_timing(self._h, int(bool(enable))), "gw_ctx_kernel_timing", self._h)

@@ -25,9 +25,22 @@ struct gw_ctx {
     int64_t      launches;
     int          force_lpp, force_chunks;   // gw_ctx_force_plan (0 = planner's choice)
     int64_t      force_ctas;       // gw_ctx_force_grid (0 = planner's choice)
+    int          cluster_finish;   // 1 (default): multi-lane aligned grids of <= 16 chunks reduce through thread-block clusters
     int64_t      plan_n[4];        // batch sizes of the cached plans (0 = empty): a sampler calls with few distinct sizes
     Plan         plan_of[4];       // make_plan is a pure function of n_prop for a given context and pinned shape
     int          plan_next;
+    // Small synchronous host calls (gw_lnl_batch_host, n_prop <= kHostGraphMax) replay a library-owned CUDA graph of the two
+    // kernels: theta goes through a pinned, mapped staging buffer that the setup kernel reads in place, lnL and parts come
+    // back through pinned, mapped buffers the finish stage stores to, so the call is one graph launch and one synchronise.
+    double      *pin_theta, *pin_lnl, *pin_parts;        // host addresses (cudaHostAlloc, mapped)
+    double      *pin_theta_dev, *pin_lnl_dev, *pin_parts_dev;
+    int64_t      pin_cap;                                 // proposals the pinned buffers hold
+    cudaStream_t capture_stream;                          // graphs are captured here and launched on the caller's stream
+    int64_t      graph_n[4];       // batch size of a cached graph (0 = empty), with or without parts
+    int          graph_parts[4];
+    cudaGraphExec_t graph_exec[4];
+    int          graph_next;
+    int          host_graph;       // 1 (default): use the graph path; gw_ctx_host_graph switches it
     int          timing;           // gw_ctx_kernel_timing: record events around K1 and the main kernel
     cudaEvent_t  ev[3];            // before K1, between K1 and main, after main
 };
@@ -35,6 +48,10 @@ struct gw_ctx {
 namespace {
 
 constexpr int64_t kHStageMaxDoubles = (int64_t)1 << 26;       // 512 MiB waveform slab for the host variant
+#ifndef GW_HOST_GRAPH_MAX
+#define GW_HOST_GRAPH_MAX 512
+#endif
+constexpr int64_t kHostGraphMax = GW_HOST_GRAPH_MAX;          // largest batch the host variant sends through its graph
 
 int cuda_fail(gw_ctx *ctx, cudaError_t e)
 {
@@ -91,6 +108,14 @@ constexpr int64_t kMaxWaves = 8;
 #endif
 constexpr double kMultiPenalty = GW_MULTI_PENALTY;     // the lanes-interleaved loop costs this much more per bin (measured, C2)
 constexpr double kTwoLevelHop = 16.0;      // the second fence + ticket round of the two-level finish (~2 us; C4 B = 1, 16)
+#ifndef GW_CLUSTER_FINISH_COST
+#define GW_CLUSTER_FINISH_COST 4.0
+#endif
+#ifndef GW_CLUSTER_MAX_CTAS
+#define GW_CLUSTER_MAX_CTAS 32
+#endif
+constexpr int64_t kClusterMaxCtas = GW_CLUSTER_MAX_CTAS;    // grids up to this many CTAs may be launched as clusters
+constexpr double kClusterFinish = GW_CLUSTER_FINISH_COST;   // cluster barrier + one distributed-shared-memory round trip, in bin sweeps
 constexpr double kFinishPerChunk = 1.0;    // serial additions of the finish stage, in bin-sweep equivalents each (calibrated on C4 B = 256, 512)
 
 // exact maximum of segments per tile for a grid of n_cta CTAs over n_tiles tiles of M bins
@@ -112,7 +137,8 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
     const int slots_per_sm = ctx->ctas_per_sm > 0 ? ctx->ctas_per_sm : 1;
     const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 148;
     const int64_t slots = (int64_t)n_sm * slots_per_sm;
-    Plan best = {1, kThreads, (n_prop + kThreads - 1) / kThreads, (n_prop + kThreads - 1) / kThreads, 1, 1, 0};
+    Plan best = {1, kThreads, (n_prop + kThreads - 1) / kThreads, (n_prop + kThreads - 1) / kThreads, 1, 1, 0, 0};
+    const int64_t stage_doubles = (int64_t)kStages * (kBasisPlanes + ctx->t.n_det) * kStageBins * 2;   // a CTA's idle stage ring
     double best_cost = 1e300;
     for (int lpp = 1; lpp <= 32; lpp *= 2) {
         if (ctx->force_lpp > 0 && lpp != ctx->force_lpp) continue;
@@ -155,7 +181,14 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
             double slowdown = warps_per_sched > kSatWarps ? warps_per_sched / kSatWarps : 1.0;
             if (resident >= 2.0) slowdown *= (lpp > 1 ? kCoResidentGainMulti : kCoResidentGain);  // a second CTA hides the first one's stage boundaries
             const int64_t nseg = aligned ? ctas / tiles : (ctas + tiles - 1) / tiles + 1;   // segments per tile
-            const double finish_len = nseg >= kFinishTwoLevelFrom ? kTwoLevelHop + (double)(kFinishGroup + (nseg + kFinishGroup - 1) / kFinishGroup)
+            // Multi-lane aligned grids of 2..16 chunks per tile launch every tile as one thread-block cluster and reduce the
+            // chunk sums through distributed shared memory (no global partials, fence or ticket): a short, flat finish.
+            // Only for grids of a few clusters: many clusters of 9-16 CTAs wait for whole groups of free SMs in one GPC
+            // (measured: B = 64, 256 and C0 lose 5-9 us with clusters, B = 1 and 16 gain 2 us).
+            const bool clustered = ctx->cluster_finish && lpp > 1 && aligned && nseg >= 2 && nseg <= kMaxCluster && ctas <= kClusterMaxCtas &&
+                                   (int64_t)(2 * ctx->t.n_det) * pt * (nseg + 1) <= stage_doubles;
+            const double finish_len = clustered ? kClusterFinish
+                                    : nseg >= kFinishTwoLevelFrom ? kTwoLevelHop + (double)(kFinishGroup + (nseg + kFinishGroup - 1) / kFinishGroup)
                                                                   : (double)nseg;   // serial additions of the finish
             // lanes-interleaved CTAs have short sweeps and a latency-bound prologue that a co-resident CTA covers
             const double per_cta = lpp > 1 ? sweep * slowdown + pro : (sweep + pro) * slowdown;
@@ -166,6 +199,7 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
                 best.lpp = lpp; best.props_per_cta = pt; best.n_cta = ctas; best.n_tiles = tiles;
                 // a grid that fits one CTA per SM is launched so that no SM takes two (launch_fused)
                 best.exclusive = (GW_EXCLUSIVE_PLANS && ctas <= n_sm) ? 1 : 0;
+                best.cluster = clustered ? (int)nseg : 0;
             }
         }
         if (tiles >= slots && ctx->force_lpp == 0) break;     // enough proposals to fill the GPU: keep this lpp
@@ -173,6 +207,15 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
     best.max_seg = max_segments_per_tile(best.n_tiles, M, best.n_cta);
     best.gmax = best.max_seg >= kFinishTwoLevelFrom ? (best.max_seg + kFinishGroup - 1) / kFinishGroup : 1;
     return best;
+}
+
+void drop_host_graphs(gw_ctx *ctx)
+{
+    for (int i = 0; i < 4; ++i) {
+        if (ctx->graph_exec[i]) cudaGraphExecDestroy(ctx->graph_exec[i]);
+        ctx->graph_exec[i] = nullptr;
+        ctx->graph_n[i] = 0;
+    }
 }
 
 // make_plan through a four-entry cache (the planner's search costs several microseconds of host time per call)
@@ -199,7 +242,7 @@ int64_t partial_bound(const gw_ctx *ctx, int64_t max_batch)
 
 int64_t partial_need(const gw_ctx *ctx, const Plan &p)
 {
-    return p.max_seg > 1 ? plan_partial_slots(p) * (int64_t)(2 * ctx->t.n_det) * p.props_per_cta : 0;
+    return (p.max_seg > 1 && !p.cluster) ? plan_partial_slots(p) * (int64_t)(2 * ctx->t.n_det) * p.props_per_cta : 0;
 }
 
 void free_workspace(Workspace &w)
@@ -245,6 +288,7 @@ int reserve_impl(gw_ctx *ctx, int64_t max_batch)
         cudaGetLastError();
         return cuda_fail(ctx, e);
     }
+    drop_host_graphs(ctx);                                   // cached graphs hold pointers into the old workspace
     double *old_h = ctx->w.h_stage;
     const int64_t old_h_doubles = ctx->w.h_stage_doubles;
     ctx->w.h_stage = nullptr;
@@ -356,6 +400,7 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
     ctx->device = dev;
     ctx->n_sm = prop.multiProcessorCount;
     ctx->spin_order = o.spin_order;
+    ctx->cluster_finish = 1;
     ctx->gmst = gmst_rad;
     for (int i = 0; i < n_det; ++i) {
         const gw_detector &d = dets[i];
@@ -403,6 +448,19 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
         if ((e = cudaMemcpyAsync(t.i7, di7, sizeof(double) * n_det, cudaMemcpyDeviceToHost, s)) != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
         rc = reserve_impl(ctx, o.max_batch);
+        if (rc != GW_OK) break;
+        // pinned, mapped staging of the small-batch host path (fixed size: kHostGraphMax proposals)
+        ctx->pin_cap = kHostGraphMax;
+        ok = true;
+        ok = ok && (e = cudaHostAlloc(&ctx->pin_theta, sizeof(double) * ctx->pin_cap * t.n_param, cudaHostAllocMapped)) == cudaSuccess;
+        ok = ok && (e = cudaHostAlloc(&ctx->pin_lnl, sizeof(double) * ctx->pin_cap, cudaHostAllocMapped)) == cudaSuccess;
+        ok = ok && (e = cudaHostAlloc(&ctx->pin_parts, sizeof(double) * ctx->pin_cap * n_det * 3, cudaHostAllocMapped)) == cudaSuccess;
+        ok = ok && (e = cudaHostGetDevicePointer(&ctx->pin_theta_dev, ctx->pin_theta, 0)) == cudaSuccess;
+        ok = ok && (e = cudaHostGetDevicePointer(&ctx->pin_lnl_dev, ctx->pin_lnl, 0)) == cudaSuccess;
+        ok = ok && (e = cudaHostGetDevicePointer(&ctx->pin_parts_dev, ctx->pin_parts, 0)) == cudaSuccess;
+        ok = ok && (e = cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking)) == cudaSuccess;
+        if (!ok) { rc = cuda_fail(ctx, e); break; }
+        ctx->host_graph = 1;
     } while (0);
     cudaFree(dfreq); cudaFree(ddata); cudaFree(dpsd); cudaFree(di7);
     if (rc != GW_OK) {
@@ -426,6 +484,9 @@ int gw_ctx_destroy(gw_ctx *ctx)
     if (!ctx) return GW_OK;
     DeviceGuard guard(ctx);
     cudaDeviceSynchronize();
+    drop_host_graphs(ctx);
+    if (ctx->capture_stream) cudaStreamDestroy(ctx->capture_stream);
+    cudaFreeHost(ctx->pin_theta); cudaFreeHost(ctx->pin_lnl); cudaFreeHost(ctx->pin_parts);
     free_workspace(ctx->w);
     cudaFree(ctx->t.planes); cudaFree(ctx->t.i7cum);
     for (int i = 0; i < 3; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
@@ -467,6 +528,7 @@ int gw_ctx_force_plan(gw_ctx *ctx, int lanes_per_prop, int n_chunks)
     ctx->force_chunks = n_chunks;
     ctx->force_ctas = 0;
     for (int i = 0; i < 4; ++i) ctx->plan_n[i] = 0;          // cached plans were made for the previous pin
+    drop_host_graphs(ctx);
     return GW_OK;
 }
 
@@ -479,6 +541,23 @@ int gw_ctx_force_grid(gw_ctx *ctx, int lanes_per_prop, int64_t n_ctas)
     ctx->force_chunks = 0;
     ctx->force_ctas = n_ctas;
     for (int i = 0; i < 4; ++i) ctx->plan_n[i] = 0;
+    drop_host_graphs(ctx);
+    return GW_OK;
+}
+
+int gw_ctx_cluster_finish(gw_ctx *ctx, int enable)
+{
+    if (!ctx) return GW_ERR_INVALID_ARG;
+    ctx->cluster_finish = enable ? 1 : 0;
+    for (int i = 0; i < 4; ++i) ctx->plan_n[i] = 0;
+    drop_host_graphs(ctx);
+    return GW_OK;
+}
+
+int gw_ctx_host_graph(gw_ctx *ctx, int enable)
+{
+    if (!ctx) return GW_ERR_INVALID_ARG;
+    ctx->host_graph = enable ? 1 : 0;
     return GW_OK;
 }
 
@@ -595,6 +674,40 @@ int gw_lnl_batch_host(gw_ctx *ctx, int64_t n_prop, const double *theta_host, dou
     DeviceGuard guard(ctx);
     cudaStream_t s = (cudaStream_t)cuda_stream;
     Workspace &w = ctx->w;
+    if (ctx->host_graph && !ctx->timing && n_prop <= ctx->pin_cap) {
+        // Small batch: one graph launch (setup kernel reading theta in place from the pinned staging buffer, fused kernel
+        // storing lnL and parts into pinned buffers) and one synchronise.  The graph of a batch size is captured once on
+        // the library's own stream and kept (four sizes, with / without parts).
+        const int want_parts = parts_out_host != nullptr;
+        cudaGraphExec_t exec = nullptr;
+        for (int i = 0; i < 4; ++i)
+            if (ctx->graph_n[i] == n_prop && ctx->graph_parts[i] == want_parts) exec = ctx->graph_exec[i];
+        cudaError_t e;
+        if (!exec) {
+            cudaGraph_t graph = nullptr;
+            if ((e = cudaStreamBeginCapture(ctx->capture_stream, cudaStreamCaptureModeThreadLocal)) != cudaSuccess) return cuda_fail(ctx, e);
+            rc = lnl_batch_impl(ctx, n_prop, ctx->pin_theta_dev, 1, ctx->pin_lnl_dev, want_parts ? ctx->pin_parts_dev : nullptr,
+                                (void *)ctx->capture_stream);
+            e = cudaStreamEndCapture(ctx->capture_stream, &graph);
+            if (rc == GW_OK) ctx->launches -= 2;             // captured, not launched
+            if (rc != GW_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (e != cudaSuccess) return cuda_fail(ctx, e);
+            e = cudaGraphInstantiate(&exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) return cuda_fail(ctx, e);
+            const int slot = ctx->graph_next;
+            ctx->graph_next = (slot + 1) & 3;
+            if (ctx->graph_exec[slot]) cudaGraphExecDestroy(ctx->graph_exec[slot]);
+            ctx->graph_exec[slot] = exec; ctx->graph_n[slot] = n_prop; ctx->graph_parts[slot] = want_parts;
+        }
+        std::memcpy(ctx->pin_theta, theta_host, sizeof(double) * n_prop * ctx->t.n_param);
+        if ((e = cudaGraphLaunch(exec, s)) != cudaSuccess) return cuda_fail(ctx, e);
+        ctx->launches += 2;
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return cuda_fail(ctx, e);
+        std::memcpy(lnl_out_host, ctx->pin_lnl, sizeof(double) * n_prop);
+        if (want_parts) std::memcpy(parts_out_host, ctx->pin_parts, sizeof(double) * n_prop * ctx->t.n_det * 3);
+        return GW_OK;
+    }
     // A pinned theta buffer is read in place by the setup kernel (coalesced loads over the host link): one
     // copy-engine operation and its hand-over to the kernel less per call; pageable buffers and very large batches
     // (whose transfer the copy engine does faster) take the staged copy.

@@ -41,6 +41,7 @@ constexpr int kBasis      = 8;     // per-bin phase basis values (4 planes of 2)
 constexpr int kBasisPlanes = 5;    // (x^-5,x^-3) (x^-2,x^-1) (ln f,x) (x ln f,x^2) (f,f^-7/6)
 constexpr int kFinishGroup = 16;   // chunks per group of the two-level finish
 constexpr int kFinishTwoLevelFrom = 33;  // n_chunks from which the finish is two-level
+constexpr int kMaxCluster = 16;          // chunks per tile up to which they are launched as one cluster (non-portable size)
 constexpr int kExclusiveSmemBytes = 120 * 1024;   // > half of an SM's 228 KB: at most one such CTA per SM
 constexpr int kRecFixed   = 10;    // record fields before the per-detector block
 constexpr int kRecPerDet  = 5;     // tau, Cre, Cim, rot_re, rot_im
@@ -90,6 +91,7 @@ struct Plan {
     int     max_seg;      // upper bound of segments per tile (what gw_ctx_plan reports as n_chunks)
     int     gmax;         // groups per tile of the two-level finish: stride of the group workspace (>= 1)
     int     exclusive;    // 1: the grid has at most one CTA per SM and is launched so that no SM takes two
+    int     cluster;      // > 0: aligned multi-lane grid whose n_chunks (= cluster) chunks per tile form a thread-block cluster
 };
 
 // ---- flattened work ranges (shared by the kernel, the planner and the CPU tests of the host logic) --------------

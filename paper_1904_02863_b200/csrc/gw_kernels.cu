@@ -586,6 +586,7 @@ struct FusedArgs {
     int64_t n_cta;           // CTAs of the grid: CTA k sweeps [k work / n_cta, (k+1) work / n_cta)
     int     lpp;
     int     gmax;            // groups per tile of the two-level finish (stride of gpartial / gtickets)
+    int     cluster;         // > 0: the chunks of a tile are one thread-block cluster of this size (multi-lane layouts)
     double  f0, delta_f;
     double  i7[GW_MAX_DET];
     const double *i7cum;     // isco_cut: [NDET][n_pad] prefix sums of the norm
@@ -920,6 +921,47 @@ __device__ __forceinline__ void fused_segment(const FusedArgs &a, const Segment 
         if (sub == 0 && live) finish_proposal<NDET, ISCO>(a, b, load_finish_rec<NDET, ISCO>(a, b), zr, zi);
         return;
     }
+    if (MULTI && a.cluster > 0) {
+        // The n_seg chunks of this tile are one thread-block cluster (aligned grid, n_seg = cluster size <= 16): the
+        // partial sums go to each CTA's own (now idle) stage buffers, and CTA 0 of the cluster gathers them through
+        // distributed shared memory in one round trip and adds them in chunk order -- no global partials, no fence, no
+        // ticket.  Same additions in the same order as the ticket path below, so the bits are identical.
+        double *sh = reinterpret_cast<double *>(smem_raw);
+        const int blk = 2 * NDET * PT;                       // doubles per CTA
+        if (sub == 0) {
+#pragma unroll
+            for (int i = 0; i < NDET; ++i) { sh[(2 * i) * PT + pic] = zr[i]; sh[(2 * i + 1) * PT + pic] = zi[i]; }
+        }
+        const int64_t b_fin = tile * PT + (tid < PT ? tid : 0);
+        const FinishRec<NDET> frec = load_finish_rec<NDET, ISCO>(a, b_fin < a.n_prop ? b_fin : a.n_prop - 1);
+        cluster_sync();                                      // every CTA's block is in place
+        if (cluster_ctarank() == 0) {
+            double *gather = sh + blk;
+            const int nvals = blk * n_seg;
+            for (int i = tid; i < nvals; i += kThreads) gather[i] = ld_dsmem_f64(sh + (i % blk), (uint32_t)(i / blk));
+        }
+        cluster_sync();                                      // CTA 0 has read everybody's block: the others may leave
+        if (cluster_ctarank() != 0) return;
+        __syncthreads();
+        if (tid < PT) {
+            const int64_t bb = tile * PT + tid;
+            if (bb < a.n_prop) {
+                const double *gather = sh + blk;
+                double sr[NDET], si[NDET];
+#pragma unroll
+                for (int i = 0; i < NDET; ++i) { sr[i] = 0.0; si[i] = 0.0; }
+                for (int c = 0; c < n_seg; ++c) {
+#pragma unroll
+                    for (int i = 0; i < NDET; ++i) {
+                        sr[i] += gather[(c * 2 * NDET + 2 * i) * PT + tid];
+                        si[i] += gather[(c * 2 * NDET + 2 * i + 1) * PT + tid];
+                    }
+                }
+                finish_proposal<NDET, ISCO>(a, bb, frec, sr, si);
+            }
+        }
+        return;
+    }
     // stage 1 -> workspace: partial[(slot*2*NDET + comp)*PT + pic], slot = cta + tile (consecutive along the tile)
     const int64_t slot0 = seg.first_cta + tile;              // slot of the tile's first segment
     double *part = a.partial + (seg.slot * (int64_t)(2 * NDET)) * PT;
@@ -1087,10 +1129,15 @@ static cudaError_t launch_fused_t(const FusedArgs &a, int64_t blocks, bool exclu
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)blocks); cfg.blockDim = dim3(kThreads);
     cfg.dynamicSmemBytes = exclusive ? fused_smem_bytes_exclusive(NDET) : fused_smem_bytes(NDET); cfg.stream = s;
-    cudaLaunchAttribute at[1];
+    cudaLaunchAttribute at[2];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
+    if (MULTI && a.cluster > 0) {                            // the chunks of a tile form one cluster
+        at[1].id = cudaLaunchAttributeClusterDimension;
+        at[1].val.clusterDim.x = (unsigned)a.cluster; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
+        cfg.numAttrs = 2;
+    }
     return cudaLaunchKernelEx(&cfg, fused_kernel<NDET, MULTI, ISCO, TIDAL>, a);
 }
 
@@ -1101,7 +1148,7 @@ cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, cons
     FusedArgs a;
     a.planes = t.planes; a.rec = rec; a.n_pad = t.n_pad; a.n_bins = t.n_bins; a.n_prop = n_prop;
     a.rec_stride = rec_stride; a.lpp = plan.lpp; a.f0 = t.f0; a.delta_f = t.delta_f;
-    a.work = plan.n_tiles * t.n_bins; a.n_cta = plan.n_cta; a.gmax = plan.gmax;
+    a.work = plan.n_tiles * t.n_bins; a.n_cta = plan.n_cta; a.gmax = plan.gmax; a.cluster = plan.cluster;
     for (int i = 0; i < GW_MAX_DET; ++i) a.i7[i] = t.i7[i];
     a.partial = partial; a.tickets = tickets; a.lnl = lnl_out; a.parts = parts_out;
     a.gpartial = gpartial; a.gtickets = gtickets;
@@ -1147,6 +1194,10 @@ static cudaError_t configure_one()
     for (int v = 0; v < 8; ++v) {
         e = cudaFuncSetAttribute(variants[v], cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
+        if (v & 1) {                                         // multi-lane variants: clusters of up to 16 chunks
+            e = cudaFuncSetAttribute(variants[v], cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            if (e != cudaSuccess) return e;
+        }
     }
     int n = 0;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fused_kernel<NDET, false, false, false>, kThreads, fused_smem_bytes(NDET));

@@ -473,3 +473,63 @@ def test_phase_domain_guard(oracle, torch_cuda):
     assert np.isnan(lnl[1]) and np.all(np.isnan(h[1])) and np.all(np.isfinite(lnl[[0, 2]]))
     ref = oracle.lnl(f, 1 / 16.0, d, S, dets, 0.0, th[[0, 2]], 0)
     assert_lnl_close(lnl[[0, 2]], parts[[0, 2]], ref[0], ref[1])
+
+
+@pytest.mark.parametrize("n_det", [1, 3, 4])
+@pytest.mark.parametrize("lpp,n_chunks,batch", [(32, 16, 1), (32, 9, 20), (32, 2, 300), (16, 16, 40), (8, 5, 70), (4, 7, 130),
+                                               (2, 3, 200), (32, 17, 5)])
+def test_cluster_finish_matches_ticket_finish_bit_for_bit(oracle, torch_cuda, n_det, lpp, n_chunks, batch):
+    """Small multi-lane grids reduce the chunk sums of a tile through a thread-block cluster and distributed shared
+    memory (gw_ctx_cluster_finish, default on); the ticket path through global partial sums adds the same numbers in
+    the same order.  Both against the oracle, and against each other bit for bit; 17 chunks exceed the cluster size
+    and fall back to the ticket path by themselves."""
+    torch = torch_cuda
+    from paper_1904_02863_b200 import GwContext
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=420.0, batch=300)
+    f, S, dets_all, d_all, th = make_problem(oracle, cfg)
+    if n_det == 4:
+        dets = np.concatenate([dets_all, inputs.fixed_detector(0.4, -0.3, 0.002)[None]])
+        d = np.concatenate([d_all, d_all[:1] * 0.7])
+        S4 = np.concatenate([S, S[:1]])
+    else:
+        dets, d, S4 = dets_all[:n_det], d_all[:n_det], S[:n_det]
+    thd = _dev(torch, th[:batch])
+    with GwContext(f, d, S4, dets, cfg.gmst, spin_order=cfg.spin_order, max_batch=batch) as ctx:
+        ctx.force_plan(lpp, n_chunks)
+        a_lnl, a_parts = ctx.lnl_batch(thd, want_parts=True)
+        a2, _ = ctx.lnl_batch(thd, want_parts=True)
+        ctx.cluster_finish(False)
+        b_lnl, b_parts = ctx.lnl_batch(thd, want_parts=True)
+        torch.cuda.synchronize()
+    assert torch.equal(a_lnl, b_lnl) and torch.equal(a_parts, b_parts) and torch.equal(a_lnl, a2)
+    ref = oracle.lnl(f, cfg.delta_f, d, S4, dets, cfg.gmst, th[:batch], cfg.spin_order)
+    assert_lnl_close(a_lnl.cpu().numpy(), a_parts.cpu().numpy(), ref[0], ref[1])
+
+
+@pytest.mark.parametrize("batch", [1, 16, 300, 512, 513])
+def test_host_variant_graph_path_matches_launch_by_launch(oracle, torch_cuda, batch):
+    """gw_lnl_batch_host sends batches of up to 512 proposals through a library-owned CUDA graph (pinned staging in and
+    out, one launch per call): same bits as the launch-by-launch path and as the device variant, fresh theta on every
+    replay, with and without parts, pageable and pinned caller buffers; 513 proposals take the other path by themselves."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=260.0, batch=513)
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    th = th[:batch]
+    with make_ctx(cfg, f, d, S, dets, max_batch=batch) as ctx:
+        dev_lnl, dev_parts = ctx.lnl_batch(_dev(torch, th), want_parts=True)
+        torch.cuda.synchronize()
+        n0 = ctx.launch_count()
+        g_lnl, g_parts = ctx.lnl_batch_host(th, want_parts=True)
+        g_only = ctx.lnl_batch_host(th)
+        assert ctx.launch_count() == n0 + 4
+        th2 = th[::-1].copy()                                   # a replay of the cached graph must read the new theta
+        g_rev = ctx.lnl_batch_host(th2)
+        pin_in = torch.from_numpy(th).pin_memory().numpy()
+        pin_out = torch.empty(batch, dtype=torch.float64).pin_memory().numpy()
+        ctx.lnl_batch_host(pin_in, out=pin_out)
+        ctx.host_graph(False)
+        p_lnl, p_parts = ctx.lnl_batch_host(th, want_parts=True)
+        p_rev = ctx.lnl_batch_host(th2)
+    assert np.array_equal(g_lnl, dev_lnl.cpu().numpy()) and np.array_equal(g_parts, dev_parts.cpu().numpy())
+    assert np.array_equal(g_lnl, p_lnl) and np.array_equal(g_parts, p_parts) and np.array_equal(g_only, g_lnl)
+    assert np.array_equal(g_rev, g_lnl[::-1]) and np.array_equal(p_rev, g_rev) and np.array_equal(pin_out, g_lnl)
