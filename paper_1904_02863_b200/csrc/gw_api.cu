@@ -400,7 +400,6 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
     ctx->device = dev;
     ctx->n_sm = prop.multiProcessorCount;
     ctx->spin_order = o.spin_order;
-    ctx->cluster_finish = 1;
     ctx->gmst = gmst_rad;
     for (int i = 0; i < n_det; ++i) {
         const gw_detector &d = dets[i];
@@ -432,6 +431,7 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
     do {
         if ((e = configure_kernels(nullptr)) != cudaSuccess) { rc = cuda_fail(ctx, e); break; }
         ctx->ctas_per_sm = fused_ctas_per_sm(n_det);
+        ctx->cluster_finish = fused_cluster_ok(n_det);
         bool ok = true;
         ok = ok && (e = cudaMalloc(&t.planes, sizeof(double) * 2 * (kBasisPlanes + n_det) * t.n_pad)) == cudaSuccess;
         if (t.isco_cut) ok = ok && (e = cudaMalloc(&t.i7cum, sizeof(double) * n_det * t.n_pad)) == cudaSuccess;
@@ -548,7 +548,7 @@ int gw_ctx_force_grid(gw_ctx *ctx, int lanes_per_prop, int64_t n_ctas)
 int gw_ctx_cluster_finish(gw_ctx *ctx, int enable)
 {
     if (!ctx) return GW_ERR_INVALID_ARG;
-    ctx->cluster_finish = enable ? 1 : 0;
+    ctx->cluster_finish = (enable && fused_cluster_ok(ctx->t.n_det)) ? 1 : 0;
     for (int i = 0; i < 4; ++i) ctx->plan_n[i] = 0;
     drop_host_graphs(ctx);
     return GW_OK;

@@ -160,6 +160,7 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
                             double *h_out, cudaStream_t s, int64_t *launches);
 cudaError_t configure_kernels(int *fused_ctas_per_sm);      // smem attributes + occupancy query (per n_det below)
 int         fused_ctas_per_sm(int n_det);
+int         fused_cluster_ok(int n_det);       // 1: clusters of kMaxCluster fused CTAs can be scheduled on this device
 size_t      fused_smem_bytes(int n_det);
 
 } // namespace gw

@@ -1180,6 +1180,7 @@ cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, cons
 }
 
 static int g_ctas_per_sm[GW_MAX_DET + 1] = {0, 0, 0, 0, 0};
+static int g_cluster_ok[GW_MAX_DET + 1] = {0, 0, 0, 0, 0};
 
 template <int NDET>
 static cudaError_t configure_one()
@@ -1203,6 +1204,19 @@ static cudaError_t configure_one()
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fused_kernel<NDET, false, false, false>, kThreads, fused_smem_bytes(NDET));
     if (e != cudaSuccess) return e;
     g_ctas_per_sm[NDET] = n > 0 ? n : 1;
+    // can a cluster of kMaxCluster exclusive CTAs (one per SM) be co-scheduled at all on this device?
+    {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(kMaxCluster); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = (size_t)smem;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = kMaxCluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int n_clusters = 0;
+        const cudaError_t ec = cudaOccupancyMaxActiveClusters(&n_clusters, fused_kernel<NDET, true, false, false>, &cfg);
+        if (ec != cudaSuccess) cudaGetLastError();
+        g_cluster_ok[NDET] = (ec == cudaSuccess && n_clusters > 0) ? 1 : 0;
+    }
     return cudaSuccess;
 }
 
@@ -1218,5 +1232,6 @@ cudaError_t configure_kernels(int *out)
     return cudaSuccess;
 }
 int fused_ctas_per_sm(int n_det) { return (n_det >= 1 && n_det <= GW_MAX_DET) ? g_ctas_per_sm[n_det] : 0; }
+int fused_cluster_ok(int n_det) { return (n_det >= 1 && n_det <= GW_MAX_DET) ? g_cluster_ok[n_det] : 0; }
 
 } // namespace gw
