@@ -49,7 +49,7 @@
 extern "C" {
 #endif
 
-#define GW_ABI_VERSION 4
+#define GW_ABI_VERSION 5
 
 enum {
     GW_OK              =  0,
@@ -103,7 +103,8 @@ enum { GW_P_MC = 0, GW_P_Q, GW_P_CHI1, GW_P_CHI2, GW_P_DL, GW_P_TC, GW_P_PHIC,
  * "[n_prop][gw_ctx_n_param(ctx)]" for such a context.                                                      */
 enum { GW_P_LAMBDA1 = 11, GW_P_LAMBDA2 = 12, GW_NPARAM_TIDAL = 13 };
 
-#define GW_MAX_DET 4             /* detectors per context (the fused kernel is specialised per count)    */
+#define GW_MAX_DET 8             /* detectors per context (the fused kernel is specialised per count; 1..4 keep two
+                                  * CTAs per SM, 5..8 run one CTA per SM with the larger register budget)       */
 
 typedef struct gw_ctx gw_ctx;    /* opaque */
 

@@ -15,7 +15,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 NPARAM = 11
-MAX_DET = 4
+MAX_DET = 8
 DET_ROW = 13   # inputs.py detector row: kind, vertex[3], xarm[3], yarm[3], fplus, fcross, dt
 
 GW_OK, GW_ERR_INVALID_ARG, GW_ERR_ALLOC, GW_ERR_CUDA, GW_ERR_ARCH = 0, -1, -2, -3, -4

@@ -555,6 +555,10 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
     case 2: return tidal ? launch_waveform_t<2, true>(a, blocks, s) : launch_waveform_t<2, false>(a, blocks, s);
     case 3: return tidal ? launch_waveform_t<3, true>(a, blocks, s) : launch_waveform_t<3, false>(a, blocks, s);
     case 4: return tidal ? launch_waveform_t<4, true>(a, blocks, s) : launch_waveform_t<4, false>(a, blocks, s);
+    case 5: return tidal ? launch_waveform_t<5, true>(a, blocks, s) : launch_waveform_t<5, false>(a, blocks, s);
+    case 6: return tidal ? launch_waveform_t<6, true>(a, blocks, s) : launch_waveform_t<6, false>(a, blocks, s);
+    case 7: return tidal ? launch_waveform_t<7, true>(a, blocks, s) : launch_waveform_t<7, false>(a, blocks, s);
+    case 8: return tidal ? launch_waveform_t<8, true>(a, blocks, s) : launch_waveform_t<8, false>(a, blocks, s);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -976,7 +980,7 @@ __device__ __forceinline__ void fused_segment(const FusedArgs &a, const Segment 
     // Loads of kFinishBatch entries are issued together (the sum is latency-bound on L2 otherwise); the additions
     // stay in index order, so the result does not depend on the batching.
     auto ordered_sum = [&](const double *base, int count, double (&sr)[NDET], double (&si)[NDET]) {
-        constexpr int kFinishBatch = 8;
+        constexpr int kFinishBatch = NDET <= 4 ? 8 : 2;       // 2 * NDET * kFinishBatch doubles in flight per thread
         for (int c = 0; c < count; c += kFinishBatch) {
             // the last batch may be short: its loads are clamped to the last entry and its additions masked, so that
             // a remainder costs one round trip to L2 like a full batch (the finish is a chain of L2 latencies)
@@ -1081,7 +1085,7 @@ __device__ __forceinline__ void fused_segment(const FusedArgs &a, const Segment 
 }
 
 template <int NDET, bool MULTI, bool ISCO, bool TIDAL>
-__global__ void __launch_bounds__(kThreads, kMinCtas) fused_kernel(const FusedArgs a)
+__global__ void __launch_bounds__(kThreads, NDET > 4 ? 1 : kMinCtas) fused_kernel(const FusedArgs a)
 {
     constexpr int NP = kBasisPlanes + NDET;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -1174,13 +1178,17 @@ cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, cons
     case 2: GW_DISPATCH(2)
     case 3: GW_DISPATCH(3)
     case 4: GW_DISPATCH(4)
+    case 5: GW_DISPATCH(5)
+    case 6: GW_DISPATCH(6)
+    case 7: GW_DISPATCH(7)
+    case 8: GW_DISPATCH(8)
     default: return cudaErrorInvalidValue;
     }
 #undef GW_DISPATCH
 }
 
-static int g_ctas_per_sm[GW_MAX_DET + 1] = {0, 0, 0, 0, 0};
-static int g_cluster_ok[GW_MAX_DET + 1] = {0, 0, 0, 0, 0};
+static int g_ctas_per_sm[GW_MAX_DET + 1] = {0};
+static int g_cluster_ok[GW_MAX_DET + 1] = {0};
 
 template <int NDET>
 static cudaError_t configure_one()
@@ -1228,6 +1236,10 @@ cudaError_t configure_kernels(int *out)
     if ((e = configure_one<2>()) != cudaSuccess) return e;
     if ((e = configure_one<3>()) != cudaSuccess) return e;
     if ((e = configure_one<4>()) != cudaSuccess) return e;
+    if ((e = configure_one<5>()) != cudaSuccess) return e;
+    if ((e = configure_one<6>()) != cudaSuccess) return e;
+    if ((e = configure_one<7>()) != cudaSuccess) return e;
+    if ((e = configure_one<8>()) != cudaSuccess) return e;
     if (out) for (int i = 0; i <= GW_MAX_DET; ++i) out[i] = g_ctas_per_sm[i];
     return cudaSuccess;
 }

@@ -62,7 +62,7 @@ def test_every_header_is_covered():
 
 
 def test_no_compute_calls(lib):
-    assert lib.gw_abi_version() == 4
+    assert lib.gw_abi_version() == 5
     assert lib.gw_strerror(0) == b"ok" and b"invalid" in lib.gw_strerror(-1)
     assert lib.gw_ctx_destroy(None) == 0
     assert lib.gw_ctx_info(None, None, None, None, None) == -1
@@ -94,7 +94,7 @@ def test_create_rejects_bad_arguments_before_touching_cuda(lib):
     assert lib.gw_ctx_create(ctypes.byref(h), 1, fp, 1, dp, sp, det, 0.0, None, None) == binding.GW_ERR_INVALID_ARG
     assert lib.gw_ctx_create(ctypes.byref(h), f.size, None, 1, dp, sp, det, 0.0, None, None) == binding.GW_ERR_INVALID_ARG
     assert lib.gw_ctx_create(ctypes.byref(h), f.size, fp, 0, dp, sp, det, 0.0, None, None) == binding.GW_ERR_INVALID_ARG
-    assert lib.gw_ctx_create(ctypes.byref(h), f.size, fp, 5, dp, sp, det, 0.0, None, None) == binding.GW_ERR_INVALID_ARG
+    assert lib.gw_ctx_create(ctypes.byref(h), f.size, fp, 9, dp, sp, det, 0.0, None, None) == binding.GW_ERR_INVALID_ARG
     opt = binding.gw_options(1, 2, 16, 0, 0)      # isco_cut must be 0 or 1
     assert lib.gw_ctx_create(ctypes.byref(h), f.size, fp, 1, dp, sp, det, 0.0, ctypes.byref(opt), None) == binding.GW_ERR_INVALID_ARG
     assert not h

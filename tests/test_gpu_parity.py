@@ -103,13 +103,16 @@ def test_every_lane_width_and_chunking_forced(oracle, torch_cuda, lpp, n_chunks)
     assert_lnl_close(lnl, parts, lnl_ref, parts_ref)
 
 
-@pytest.mark.parametrize("n_det", [1, 2, 4])
+@pytest.mark.parametrize("n_det", [1, 2, 4, 5, 6, 7, 8])
 def test_detector_counts(oracle, torch_cuda, n_det):
-    """1, 2 and 4 detectors (mixed GEOMETRIC / FIXED with a non-zero fixed delay)."""
+    """1 ... GW_MAX_DET = 8 detectors (mixed GEOMETRIC / FIXED with non-zero fixed delays of both signs): lnL, parts
+    and the waveform against the oracle; counts above 4 run the one-CTA-per-SM kernel variants."""
     torch = torch_cuda
     base = inputs.CONFIGS["C1"].reduced(f_max=150.0, batch=40)
     rows = [inputs.geometric_detector("H1"), inputs.fixed_detector(0.6, -0.3, 0.0123),
-            inputs.geometric_detector("V1"), inputs.geometric_detector("L1")][:n_det]
+            inputs.geometric_detector("V1"), inputs.geometric_detector("L1"),
+            inputs.fixed_detector(-0.2, 0.7, -0.0071), inputs.geometric_detector("H1"),
+            inputs.fixed_detector(0.35, 0.35, 0.0), inputs.geometric_detector("V1")][:n_det]
     dets = np.stack(rows)
     f = inputs.frequency_grid(base)
     S = np.tile(inputs.analytic_psd(f), (n_det, 1))
@@ -307,7 +310,7 @@ def test_edge_cases_and_errors(oracle, torch_cuda):
     with pytest.raises(GwError):
         GwContext(f, d, S, skew, cfg.gmst)
     with pytest.raises(GwError):
-        GwContext(f, d[:2], S[:2], np.tile(dets[:1], (5, 1)), cfg.gmst)      # 5 detectors > GW_MAX_DET
+        GwContext(f, d[:2], S[:2], np.tile(dets[:1], (9, 1)), cfg.gmst)      # 9 detectors > GW_MAX_DET
 
 
 def test_time_shift_interchange(oracle, torch_cuda):
@@ -475,7 +478,7 @@ def test_phase_domain_guard(oracle, torch_cuda):
     assert_lnl_close(lnl[[0, 2]], parts[[0, 2]], ref[0], ref[1])
 
 
-@pytest.mark.parametrize("n_det", [1, 3, 4])
+@pytest.mark.parametrize("n_det", [1, 3, 4, 6, 8])
 @pytest.mark.parametrize("lpp,n_chunks,batch", [(32, 16, 1), (32, 9, 20), (32, 2, 300), (16, 16, 40), (8, 5, 70), (4, 7, 130),
                                                (2, 3, 200), (32, 17, 5)])
 def test_cluster_finish_matches_ticket_finish_bit_for_bit(oracle, torch_cuda, n_det, lpp, n_chunks, batch):
@@ -487,10 +490,12 @@ def test_cluster_finish_matches_ticket_finish_bit_for_bit(oracle, torch_cuda, n_
     from paper_1904_02863_b200 import GwContext
     cfg = inputs.CONFIGS["C1"].reduced(f_max=420.0, batch=300)
     f, S, dets_all, d_all, th = make_problem(oracle, cfg)
-    if n_det == 4:
-        dets = np.concatenate([dets_all, inputs.fixed_detector(0.4, -0.3, 0.002)[None]])
-        d = np.concatenate([d_all, d_all[:1] * 0.7])
-        S4 = np.concatenate([S, S[:1]])
+    if n_det >= 4:
+        extra = n_det - 3
+        dets = np.concatenate([dets_all] + [inputs.fixed_detector(0.4 - 0.1 * k, -0.3 + 0.1 * k, 0.002 * (k + 1))[None]
+                                            for k in range(extra)])
+        d = np.concatenate([d_all] + [d_all[k % 3:k % 3 + 1] * (0.7 + 0.05 * k) for k in range(extra)])
+        S4 = np.concatenate([S] + [S[k % 3:k % 3 + 1] for k in range(extra)])
     else:
         dets, d, S4 = dets_all[:n_det], d_all[:n_det], S[:n_det]
     thd = _dev(torch, th[:batch])
