@@ -89,6 +89,45 @@ int64_t gw_pop_ctx_launch_count(const gw_pop_ctx *ctx);
 int gw_pop_ctx_kernel_timing(gw_pop_ctx *ctx, int enable);
 int gw_pop_ctx_last_kernel_ms(gw_pop_ctx *ctx, double *setup_ms, double *main_ms, double *finish_ms);
 
+/* ---- The no-allocation entry point ---------------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): Eq. 3 for a batch of Lambda straight from device-resident samples, WITHOUT a context.  gw_pop_lnl_static calls
+ * no cudaMalloc, cudaFree or other allocating routine, never synchronises and never copies between host and device:
+ * it enqueues one 256-byte memset and five kernels on `cuda_stream` -- the kernels of gw_pop_lnl_batch (precompute,
+ * setup, map-reduce, finish: same grids, same summation order, so the same bits) plus a one-line flag check.  All of
+ * its scratch -- the 8 per-sample planes, the Lambda records, the first-stage partial sums, the bad-sample flag -- lives
+ * in ONE file-scope `static __device__` array of GW_POP_STATIC_SCRATCH_DOUBLES doubles (16 MiB) inside the library;
+ * every GPU that loads the library holds that array until the process exits.
+ *   samples_dev  [N][n][GW_POP_NTHETA] dev (same domain as gw_pop_ctx_create);  prior_dev  [N][n] dev
+ *   lambda_dev   [n_lambda][GW_POP_NLAMBDA] dev;  lnl_out_dev  [n_lambda] dev
+ *   All four must be device memory of the CURRENT device; the caller owns them and keeps them alive until the stream
+ *   has run the call.
+ * Limit: gw_pop_static_need(N, n, n_lambda) = 32 + r32(16 n_lambda) + r32(n_lambda N ceil(n / 1024)) + 8 N n doubles
+ * (r32 rounds up to a multiple of 32) must not exceed GW_POP_STATIC_SCRATCH_DOUBLES: about 2.6e5 samples in total
+ * (PAPER.md:119's GWTC-1 catalogue of 10 x 20000 fits with 64 Lambda; PAPER.md:115's 4e6 samples do not -- use a
+ * context).  A larger problem is rejected with GW_POP_ERR_TOO_LARGE before anything is enqueued.
+ * Samples cannot be validated on the host without a synchronisation: if any sample or prior value is outside the
+ * documented domain, every lnL of that call is NaN (gw_pop_ctx_create returns GW_ERR_INVALID_ARG instead).
+ * The array is shared by every call on a device and keeps the last call's contents.  Nothing in it has to survive
+ * between calls; the one word that must start at zero (the bad-sample flag) is cleared by the call itself.  Calls
+ * enqueued on ONE stream are ordered and safe; calls that overlap on the GPU (different streams, or different host
+ * threads on different streams) RACE on the array and return garbage -- serialise them.  The first call on each
+ * device looks up the array's device address (once per device; make that call outside stream capture).
+ * Errors: GW_ERR_INVALID_ARG (NULL, bad size, a pointer that is not device memory of the current device),
+ * GW_POP_ERR_TOO_LARGE, GW_ERR_ARCH, GW_ERR_CUDA (gw_pop_static_last_cuda_error has the cudaError).
+ * n_lambda == 0 is GW_OK and enqueues nothing.                                                              */
+#define GW_POP_STATIC_SCRATCH_DOUBLES 2097152      /* 16 MiB per GPU                                          */
+#define GW_POP_ERR_TOO_LARGE (-16)                 /* the problem needs more scratch than the static array has  */
+int gw_pop_lnl_static(int64_t n_events, int64_t n_samples, const double *samples_dev, const double *prior_dev,
+                      int64_t n_lambda, const double *lambda_dev, double *lnl_out_dev, void *cuda_stream);
+
+/* Doubles of static scratch a problem of this size needs (host arithmetic only), or -1 for sizes that
+ * gw_pop_lnl_static rejects as GW_ERR_INVALID_ARG (N < 1, n < 1, n_lambda < 0 or > 2^24, N n > 4e9).          */
+int64_t gw_pop_static_need(int64_t n_events, int64_t n_samples, int64_t n_lambda);
+
+/* cudaError of the most recent GW_ERR_CUDA return of gw_pop_lnl_static in this process (0 if none).         */
+int gw_pop_static_last_cuda_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -21,6 +21,7 @@
 // conversion-pipe range reduction, degree-11 Horner -- measured 15 % SLOWER than libdevice's exp here: DESIGN.md section 13.)
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -450,6 +451,141 @@ int gw_pop_lnl_batch_host(gw_pop_ctx *ctx, int64_t n_lambda, const double *lambd
     e = cudaMemcpyAsync(lnl_out_host, ctx->lnl_stage, sizeof(double) * n_lambda, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     return e == cudaSuccess ? GW_OK : pop_fail(ctx, e);
+}
+
+} // extern "C"
+
+// =====================================================================================================================
+// The no-allocation entry point (include/gwpop.h: gw_pop_lnl_static).  Same kernels, same grids and the same summation
+// order as gw_pop_lnl_batch; every byte of scratch lives in the file-scope array below instead of a context's
+// cudaMalloc'ed workspace.  This section calls no cudaMalloc / cudaFree / allocating routine and never synchronises.
+// =====================================================================================================================
+
+// Layout (doubles): [0, 32) flag block (word 0: the bad-sample flag, cleared by every call) | Lambda records
+// [n_lambda][kRec] | partial sums [n_lambda][N][cpe] | planes [kPlanes][N n]; each part starts on a multiple of 32 doubles.
+// Every GPU that loads the library holds these 16 MiB until the process exits; every call on a device shares them.
+static __device__ __align__(256) double g_pop_static_scratch[GW_POP_STATIC_SCRATCH_DOUBLES];
+
+namespace gwpop {
+
+// a bad sample or prior value (flag set by pop_precompute_kernel) makes every lnL of the call NaN
+__global__ void pop_static_poison_kernel(int64_t n_lambda, const int *__restrict__ bad, double *__restrict__ lnl)
+{
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < n_lambda && *bad != 0) lnl[b] = __longlong_as_double(0x7ff8000000000000LL);
+}
+
+} // namespace gwpop
+
+namespace {
+
+constexpr int     kStaticFlagDoubles = 32;
+constexpr int     kStaticMaxDevices  = 64;
+constexpr int64_t kStaticCapacity    = GW_POP_STATIC_SCRATCH_DOUBLES;
+
+// In host code `g_pop_static_scratch` is a host-side stand-in for the symbol, not a device address: the address the
+// kernels may use comes from cudaGetSymbolAddress, looked up once per device with that device current.
+std::mutex g_static_mutex;
+double    *g_static_addr[kStaticMaxDevices];      // nullptr: this device has not been set up yet
+int        g_static_last_cuda_error = 0;
+
+int static_fail(cudaError_t e)
+{
+    g_static_last_cuda_error = (int)e;
+    cudaGetLastError();
+    return GW_ERR_CUDA;
+}
+
+int64_t round32(int64_t x) { return (x + 31) / 32 * 32; }
+
+// `dev` is the current device
+int static_scratch_address(int dev, double **addr)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        int major = 0;
+        cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (e != cudaSuccess) return static_fail(e);
+        if (major != 10) return GW_ERR_ARCH;
+        double *p = nullptr;
+        e = cudaGetSymbolAddress((void **)&p, g_pop_static_scratch);
+        if (e != cudaSuccess) return static_fail(e);
+        if (!p) return static_fail(cudaErrorInvalidSymbol);
+        g_static_addr[dev] = p;
+    }
+    *addr = g_static_addr[dev];
+    return GW_OK;
+}
+
+// device memory (or managed memory) that belongs to device `dev`
+bool device_ptr_of(const void *p, int dev)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return (at.type == cudaMemoryTypeDevice && at.device == dev) || at.type == cudaMemoryTypeManaged;
+}
+
+} // namespace
+
+extern "C" {
+
+int64_t gw_pop_static_need(int64_t n_events, int64_t n_samples, int64_t n_lambda)
+{
+    if (n_events < 1 || n_samples < 1 || n_lambda < 0 || n_lambda > (1 << 24)) return -1;
+    if ((double)n_events * (double)n_samples > 4.0e9) return -1;
+    const int64_t cpe = (n_samples + kChunk - 1) / kChunk;
+    return kStaticFlagDoubles + round32(kRec * n_lambda) + round32(n_lambda * n_events * cpe) + kPlanes * n_events * n_samples;
+}
+
+int gw_pop_static_last_cuda_error(void) { return g_static_last_cuda_error; }
+
+int gw_pop_lnl_static(int64_t n_events, int64_t n_samples, const double *samples_dev, const double *prior_dev,
+                      int64_t n_lambda, const double *lambda_dev, double *lnl_out_dev, void *cuda_stream)
+{
+    const int64_t need = gw_pop_static_need(n_events, n_samples, n_lambda);
+    if (need < 0) return GW_ERR_INVALID_ARG;
+    if (n_lambda == 0) return GW_OK;
+    if (!samples_dev || !prior_dev || !lambda_dev || !lnl_out_dev) return GW_ERR_INVALID_ARG;
+    if (need > kStaticCapacity) return GW_POP_ERR_TOO_LARGE;
+    const int64_t total = n_events * n_samples;
+    const int     cpe = (int)((n_samples + kChunk - 1) / kChunk);
+    const int64_t grid_x = n_events * cpe;
+    if (grid_x > 0x7fffffffLL) return GW_ERR_INVALID_ARG;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return static_fail(e);
+    if (dev < 0 || dev >= kStaticMaxDevices) return GW_ERR_INVALID_ARG;
+    if (!device_ptr_of(samples_dev, dev) || !device_ptr_of(prior_dev, dev) || !device_ptr_of(lambda_dev, dev) ||
+        !device_ptr_of(lnl_out_dev, dev))
+        return GW_ERR_INVALID_ARG;
+    double *base = nullptr;
+    const int rc = static_scratch_address(dev, &base);
+    if (rc != GW_OK) return rc;
+    int    *bad     = reinterpret_cast<int *>(base);
+    double *rec     = base + kStaticFlagDoubles;
+    double *partial = rec + round32(kRec * n_lambda);
+    double *planes  = partial + round32(n_lambda * n_events * cpe);
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    // the array keeps the last call's contents: the flag must start at zero; records, partial sums and planes are
+    // written in full by this call's kernels before anything reads them
+    if ((e = cudaMemsetAsync(base, 0, sizeof(double) * kStaticFlagDoubles, s)) != cudaSuccess) return static_fail(e);
+    pop_precompute_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(total, samples_dev, prior_dev, planes, bad);
+    if ((e = cudaGetLastError()) != cudaSuccess) return static_fail(e);
+    // launched without the programmatic attribute: starts after the precompute kernel has finished, so the main
+    // kernel (which may start as soon as the setup kernel runs, and loads planes before waiting for it) sees them
+    pop_setup_kernel<<<(unsigned)((n_lambda + 63) / 64), 64, 0, s>>>(n_lambda, lambda_dev, rec);
+    if ((e = cudaGetLastError()) != cudaSuccess) return static_fail(e);
+    PopArgs a;
+    a.planes = planes; a.rec = rec; a.total = total; a.n_samples = n_samples; a.n_events = n_events;
+    a.n_lambda = n_lambda; a.cpe = cpe; a.partial = partial; a.lnl = lnl_out_dev;
+    if (n_lambda == 1)      e = launch_pdl(pop_main_kernel<1>, dim3((unsigned)grid_x, 1), dim3(kThreads), s, a);
+    else if (n_lambda == 2) e = launch_pdl(pop_main_kernel<2>, dim3((unsigned)grid_x, 1), dim3(kThreads), s, a);
+    else                    e = launch_pdl(pop_main_kernel<kLamTile>, dim3((unsigned)grid_x, (unsigned)((n_lambda + kLamTile - 1) / kLamTile)), dim3(kThreads), s, a);
+    if (e != cudaSuccess) return static_fail(e);
+    if ((e = launch_pdl(pop_finish_kernel, dim3((unsigned)n_lambda), dim3(kFinThreads), s, a)) != cudaSuccess) return static_fail(e);
+    pop_static_poison_kernel<<<(unsigned)((n_lambda + 127) / 128), 128, 0, s>>>(n_lambda, bad, lnl_out_dev);
+    if ((e = cudaGetLastError()) != cudaSuccess) return static_fail(e);
+    return GW_OK;
 }
 
 } // extern "C"

@@ -16,7 +16,11 @@ NLAMBDA = 12    # alpha, m_min, m_max, lam, m_pp, sig_pp, beta_q, alpha_chi, bet
 
 # every symbol include/gwpop.h declares (tests/test_abi.py checks the library exports each)
 EXPORTS = ("gw_pop_ctx_create", "gw_pop_lnl_batch", "gw_pop_lnl_batch_host", "gw_pop_ctx_destroy", "gw_pop_ctx_info",
-           "gw_pop_ctx_launch_count", "gw_pop_ctx_kernel_timing", "gw_pop_ctx_last_kernel_ms")
+           "gw_pop_ctx_launch_count", "gw_pop_ctx_kernel_timing", "gw_pop_ctx_last_kernel_ms",
+           "gw_pop_lnl_static", "gw_pop_static_need", "gw_pop_static_last_cuda_error")
+
+STATIC_SCRATCH_DOUBLES = 2097152    # GW_POP_STATIC_SCRATCH_DOUBLES: the static device array of gw_pop_lnl_static (16 MiB)
+GW_POP_ERR_TOO_LARGE = -16
 
 _declared = False
 
@@ -36,8 +40,12 @@ def _lib():
         lib.gw_pop_ctx_launch_count.restype = i64
         lib.gw_pop_ctx_kernel_timing.argtypes = [vp, ci]
         lib.gw_pop_ctx_last_kernel_ms.argtypes = [vp, P(dbl), P(dbl), P(dbl)]
+        lib.gw_pop_lnl_static.argtypes = [i64, i64, vp, vp, i64, vp, vp, vp]
+        lib.gw_pop_static_need.argtypes = [i64, i64, i64]
+        lib.gw_pop_static_need.restype = i64
+        lib.gw_pop_static_last_cuda_error.argtypes = []
         for name in EXPORTS:
-            if name != "gw_pop_ctx_launch_count":
+            if name not in ("gw_pop_ctx_launch_count", "gw_pop_static_need"):
                 getattr(lib, name).restype = ci
         _declared = True
     return lib
@@ -138,3 +146,39 @@ class GwPopContext:
         _check(self._lib.gw_pop_lnl_batch_host(self._h, n, lam.ctypes.data, out.ctypes.data, _stream_ptr(stream)),
                "gw_pop_lnl_batch_host")
         return out
+
+
+def static_need(n_events: int, n_samples: int, n_lambda: int) -> int:
+    """gw_pop_static_need: doubles of static scratch gw_pop_lnl_static needs for this size (-1: a size it rejects)."""
+    return int(_lib().gw_pop_static_need(int(n_events), int(n_samples), int(n_lambda)))
+
+
+def lnl_static(samples, prior, lambdas, out=None, stream=None):
+    """gw_pop_lnl_static, the entry point that allocates nothing: samples [N][n][6], prior [N][n], Lambda [B][12], all
+    contiguous CUDA float64 tensors on the current device -> lnL [B] (``out`` or a new tensor -- pass ``out`` where
+    torch must not allocate either).  No context; the scratch is a static device array inside the library, shared by
+    every call: calls that overlap on the GPU race.  Asynchronous.  A problem beyond the array raises GwError with
+    code GW_POP_ERR_TOO_LARGE."""
+    import torch
+    for name, t, nd in (("samples", samples, 3), ("prior", prior, 2), ("lambdas", lambdas, 2)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.dim() == nd):
+            raise GwError(GW_ERR_INVALID_ARG, f"lnl_static {name}", f"want a contiguous CUDA float64 tensor with {nd} dimensions")
+    if samples.shape[2] != NTHETA or tuple(prior.shape) != tuple(samples.shape[:2]) or lambdas.shape[1] != NLAMBDA:
+        raise GwError(GW_ERR_INVALID_ARG, "lnl_static", "samples must be [N][n][6], prior [N][n] and lambdas [B][12]")
+    n_events, n_samples, n = int(samples.shape[0]), int(samples.shape[1]), int(lambdas.shape[0])
+    if out is None:
+        out = torch.empty(n, dtype=torch.float64, device=lambdas.device)
+    elif not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64 and out.is_contiguous()
+              and out.numel() >= n and out.device == lambdas.device):
+        raise GwError(GW_ERR_INVALID_ARG, "lnl_static out", f"want a contiguous CUDA float64 tensor of at least {n} elements")
+    lib = _lib()
+    rc = lib.gw_pop_lnl_static(n_events, n_samples, samples.data_ptr(), prior.data_ptr(), n, lambdas.data_ptr(),
+                               out.data_ptr(), _stream_ptr(stream))
+    if rc == GW_POP_ERR_TOO_LARGE:
+        raise GwError(rc, "gw_pop_lnl_static",
+                      f"{n_events} x {n_samples} samples with {n} Lambda need {static_need(n_events, n_samples, n)} doubles of "
+                      f"scratch, the static array holds {STATIC_SCRATCH_DOUBLES}: use a GwPopContext")
+    if rc == -3:
+        raise GwError(rc, "gw_pop_lnl_static", f"CUDA runtime error (cudaError {lib.gw_pop_static_last_cuda_error()})")
+    _check(rc, "gw_pop_lnl_static")
+    return out
