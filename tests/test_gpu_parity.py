@@ -332,14 +332,11 @@ def test_time_shift_interchange(oracle, torch_cuda):
     np.testing.assert_allclose(np.abs(ha), np.abs(hb), rtol=1e-12)
 
 
-@pytest.mark.parametrize("seed", range(int(os.environ.get("GW_RANDOM_SHAPES", "24"))))   # soak: GW_RANDOM_SHAPES=500
-def test_random_shapes(oracle, torch_cuda, seed):
-    """Seeded random shapes: bins 2..2500, proposals 1..700, 1..4 detectors (geometric and fixed mixed), random band,
-    resolution, mass range and options (incl. the tidal orders) -- ragged tails everywhere the launch planner can put one."""
+def _random_shape_case(oracle, torch_cuda, seed, det_lo, det_hi):
     torch = torch_cuda
     from paper_1904_02863_b200 import GwContext, GwError
     rng = np.random.Generator(np.random.PCG64(4242 + seed))
-    n_det = int(rng.integers(1, 5))
+    n_det = int(rng.integers(det_lo, det_hi + 1))
     M = int(rng.choice([2, 3, 5, 31, 33, 127, 129, 257, 640, 1000, 2500]))
     B = int(rng.choice([1, 2, 5, 8, 17, 32, 100, 255, 256, 300, 700]))
     df = float(rng.choice([1 / 128, 1 / 16, 0.125, 0.25, 1.0]))
@@ -419,6 +416,20 @@ def test_random_shapes(oracle, torch_cuda, seed):
     assert np.all(h[~nz] == 0)
     if nz.any():
         assert (np.abs(h - h_ref)[nz] / hs[nz]).max() <= 1e-9
+
+
+@pytest.mark.parametrize("seed", range(int(os.environ.get("GW_RANDOM_SHAPES", "24"))))   # soak: GW_RANDOM_SHAPES=500
+def test_random_shapes(oracle, torch_cuda, seed):
+    """Seeded random shapes: bins 2..2500, proposals 1..700, 1..4 detectors (geometric and fixed mixed), random band,
+    resolution, mass range and options (incl. the tidal orders) -- ragged tails everywhere the launch planner can put one."""
+    _random_shape_case(oracle, torch_cuda, seed, 1, 4)
+
+
+@pytest.mark.parametrize("seed", range(100, 100 + int(os.environ.get("GW_RANDOM_SHAPES_MANY_DET", "8"))))
+def test_random_shapes_five_to_eight_detectors(oracle, torch_cuda, seed):
+    """The same seeded random shapes with 5..8 detectors (the one-CTA-per-SM kernel variants)."""
+    _random_shape_case(oracle, torch_cuda, seed, 5, 8)
+
 
 
 def test_cuda_phase_against_40_digit_arithmetic(torch_cuda):
