@@ -32,10 +32,20 @@ int gw_ctx_cluster_finish(gw_ctx *ctx, int enable);
 int gw_ctx_host_graph(gw_ctx *ctx, int enable);
 
 /* Host-only (no CUDA call): the segments that CTA `cta` of a grid of n_ctas CTAs sweeps when n_tiles proposal tiles
- * of n_bins bins are shared equally -- the same arithmetic the fused kernel runs (csrc/gw_internal.h, segment_at).
+ * of n_bins bins, separated by boundary_bins positions without work (gw_ctx_boundary_bins; 0 = none), are shared
+ * equally -- the same arithmetic the fused kernel runs (csrc/gw_internal.h, segment_at).  A range that only touches
+ * boundary positions of a tile yields a row with j0 == j1 == n_bins (a segment of no bins).
  * Writes up to max_rows rows of 6 values (tile, j0, j1, index of the segment within its tile, segments of that tile,
  * partial-sum slot) and returns the number of segments of the CTA, or GW_ERR_INVALID_ARG.                     */
-int gw_plan_cta_segments(int64_t n_tiles, int64_t n_bins, int64_t n_ctas, int64_t cta, int max_rows, int64_t *rows6);
+int gw_plan_cta_segments(int64_t n_tiles, int64_t n_bins, int64_t boundary_bins, int64_t n_ctas, int64_t cta, int max_rows,
+                         int64_t *rows6);
+
+/* Testing / tuning aid: on balanced grids (n_ctas not a multiple of the tile count) consecutive tiles are separated by
+ * boundary positions without work in the flattened space, so that a CTA whose range crosses a tile boundary -- and pays
+ * a segment end and a second prologue -- sweeps that many bins less and finishes with the others (default 30 per lane;
+ * 0 = plain equal shares).  gw_ctx_plan_boundary_bins reports the value a batch size's plan uses (0 on aligned grids). */
+int gw_ctx_boundary_bins(gw_ctx *ctx, int boundary_bins);
+int gw_ctx_plan_boundary_bins(const gw_ctx *ctx, int64_t n_prop, int *boundary_bins);
 
 /* Measurement aid: when enabled, the *_batch calls record CUDA events on their stream before the setup
  * kernel, between the setup kernel and the main (fused or waveform) kernel, and after it.  The event between

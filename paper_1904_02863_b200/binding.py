@@ -27,7 +27,7 @@ EXPORTS = (
     "gw_ctx_launch_count", "gw_strerror", "gw_last_cuda_error", "gw_abi_version",
 )
 # include/gwlnl_tuning.h: testing / tuning aids exported by the same library, outside the product boundary
-TUNING_EXPORTS = ("gw_ctx_force_plan", "gw_ctx_force_grid", "gw_ctx_cluster_finish", "gw_ctx_host_graph", "gw_plan_cta_segments", "gw_ctx_kernel_timing",
+TUNING_EXPORTS = ("gw_ctx_force_plan", "gw_ctx_force_grid", "gw_ctx_cluster_finish", "gw_ctx_host_graph", "gw_ctx_boundary_bins", "gw_ctx_plan_boundary_bins", "gw_plan_cta_segments", "gw_ctx_kernel_timing",
                   "gw_ctx_last_kernel_ms")
 
 
@@ -86,7 +86,9 @@ def load_library():
     lib.gw_ctx_force_grid.argtypes = [vp, ci, i64]
     lib.gw_ctx_cluster_finish.argtypes = [vp, ci]
     lib.gw_ctx_host_graph.argtypes = [vp, ci]
-    lib.gw_plan_cta_segments.argtypes = [i64, i64, i64, i64, ci, P(i64)]
+    lib.gw_plan_cta_segments.argtypes = [i64, i64, i64, i64, i64, ci, P(i64)]
+    lib.gw_ctx_boundary_bins.argtypes = [vp, ci]
+    lib.gw_ctx_plan_boundary_bins.argtypes = [vp, i64, P(ci)]
     lib.gw_ctx_kernel_timing.argtypes = [vp, ci]
     lib.gw_ctx_last_kernel_ms.argtypes = [vp, P(dbl), P(dbl)]
     lib.gw_strerror.argtypes = [ci]
@@ -237,6 +239,15 @@ class GwContext:
         """Tuning aid: small lnl_batch_host calls through the library-owned CUDA graph (default) or launch by launch."""
         _check(self._lib.gw_ctx_host_graph(self._h, int(bool(enable))), "gw_ctx_host_graph", self._h)
 
+    def boundary_bins(self, bins: int):
+        """Tuning aid: bins (per lane) by which a range that crosses a tile boundary is shortened on balanced grids."""
+        _check(self._lib.gw_ctx_boundary_bins(self._h, int(bins)), "gw_ctx_boundary_bins", self._h)
+
+    def plan_boundary_bins(self, n_prop: int) -> int:
+        v = ctypes.c_int()
+        _check(self._lib.gw_ctx_plan_boundary_bins(self._h, int(n_prop), ctypes.byref(v)), "gw_ctx_plan_boundary_bins", self._h)
+        return v.value
+
     def kernel_timing(self, enable: bool):
         _check(self._lib.gw_ctx_kernel_timing(self._h, int(bool(enable))), "gw_ctx_kernel_timing", self._h)
 
@@ -340,16 +351,16 @@ class GwContext:
         return out
 
 
-def plan_cta_segments(n_tiles: int, n_bins: int, n_ctas: int, cta: int, max_rows: int = 64) -> np.ndarray:
+def plan_cta_segments(n_tiles: int, n_bins: int, n_ctas: int, cta: int, max_rows: int = 64, boundary_bins: int = 0) -> np.ndarray:
     """gw_plan_cta_segments (host only): rows (tile, j0, j1, index, count, slot) of the segments one CTA sweeps."""
     lib = load_library()
     rows = np.zeros((max_rows, 6), dtype=np.int64)
-    n = lib.gw_plan_cta_segments(int(n_tiles), int(n_bins), int(n_ctas), int(cta), int(max_rows),
+    n = lib.gw_plan_cta_segments(int(n_tiles), int(n_bins), int(boundary_bins), int(n_ctas), int(cta), int(max_rows),
                                  rows.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)))
     if n < 0:
         raise GwError(n, "gw_plan_cta_segments", "invalid argument")
     if n > max_rows:
-        return plan_cta_segments(n_tiles, n_bins, n_ctas, cta, n)
+        return plan_cta_segments(n_tiles, n_bins, n_ctas, cta, n, boundary_bins)
     return rows[:n]
 
 

@@ -41,6 +41,7 @@ struct gw_ctx {
     cudaGraphExec_t graph_exec[4];
     int          graph_next;
     int          host_graph;       // 1 (default): use the graph path; gw_ctx_host_graph switches it
+    int          boundary_bins;    // per lane: bins a range that crosses a tile boundary is shortened by on balanced grids (gw_ctx_boundary_bins)
     int          timing;           // gw_ctx_kernel_timing: record events around K1 and the main kernel
     cudaEvent_t  ev[3];            // before K1, between K1 and main, after main
 };
@@ -116,16 +117,21 @@ constexpr double kTwoLevelHop = 16.0;      // the second fence + ticket round of
 #endif
 constexpr int64_t kClusterMaxCtas = GW_CLUSTER_MAX_CTAS;    // grids up to this many CTAs may be launched as clusters
 constexpr double kClusterFinish = GW_CLUSTER_FINISH_COST;   // cluster barrier + one distributed-shared-memory round trip, in bin sweeps
+#ifndef GW_BOUNDARY_BINS
+#define GW_BOUNDARY_BINS 30
+#endif
+constexpr int kBoundaryBins = GW_BOUNDARY_BINS;   // a segment end plus a second prologue, in bin sweeps of a one-lane CTA (timeline of C1: 3.3-3.8 us at 0.12 us per bin)
 constexpr double kFinishPerChunk = 1.0;    // serial additions of the finish stage, in bin-sweep equivalents each (calibrated on C4 B = 256, 512)
 
 // exact maximum of segments per tile for a grid of n_cta CTAs over n_tiles tiles of M bins
-int max_segments_per_tile(int64_t n_tiles, int64_t M, int64_t n_cta)
+int max_segments_per_tile(int64_t n_tiles, int64_t M, int64_t vbins, int64_t n_cta)
 {
-    const int64_t work = n_tiles * M;
-    if (n_cta % n_tiles == 0) return (int)(n_cta / n_tiles);           // aligned grid: every tile in n_cta / n_tiles chunks
+    const int64_t L = M + vbins, work = flattened_work(n_tiles, M, vbins);
+    if (vbins == 0 && n_cta % n_tiles == 0) return (int)(n_cta / n_tiles);   // aligned grid: every tile in n_cta / n_tiles chunks
     int64_t best = 1;
     for (int64_t t = 0; t < n_tiles; ++t) {
-        const int64_t c = cta_of_position(t * M + M - 1, work, n_cta) - cta_of_position(t * M, work, n_cta) + 1;
+        const int64_t t_end = t * L + L < work ? t * L + L : work;            // boundary positions belong to the tile (segment_at)
+        const int64_t c = cta_of_position(t_end - 1, work, n_cta) - cta_of_position(t * L, work, n_cta) + 1;
         if (c > best) best = c;
     }
     return (int)best;
@@ -137,7 +143,7 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
     const int slots_per_sm = ctx->ctas_per_sm > 0 ? ctx->ctas_per_sm : 1;
     const int n_sm = ctx->n_sm > 0 ? ctx->n_sm : 148;
     const int64_t slots = (int64_t)n_sm * slots_per_sm;
-    Plan best = {1, kThreads, (n_prop + kThreads - 1) / kThreads, (n_prop + kThreads - 1) / kThreads, 1, 1, 0, 0};
+    Plan best = {1, kThreads, (n_prop + kThreads - 1) / kThreads, (n_prop + kThreads - 1) / kThreads, 1, 1, 0, 0, 0};
     const int64_t stage_doubles = (int64_t)kStages * (kBasisPlanes + ctx->t.n_det) * kStageBins * 2;   // a CTA's idle stage ring
     double best_cost = 1e300;
     for (int lpp = 1; lpp <= 32; lpp *= 2) {
@@ -200,11 +206,13 @@ Plan make_plan(const gw_ctx *ctx, int64_t n_prop)
                 // a grid that fits one CTA per SM is launched so that no SM takes two (launch_fused)
                 best.exclusive = (GW_EXCLUSIVE_PLANS && ctas <= n_sm) ? 1 : 0;
                 best.cluster = clustered ? (int)nseg : 0;
+                // ranges that cross a tile boundary get vbins bins less (gw_internal.h, segment_at); aligned grids have none
+                best.vbins = (aligned || tiles < 2 || work / ctas < 4 * (int64_t)ctx->boundary_bins * lpp) ? 0 : ctx->boundary_bins * lpp;
             }
         }
         if (tiles >= slots && ctx->force_lpp == 0) break;     // enough proposals to fill the GPU: keep this lpp
     }
-    best.max_seg = max_segments_per_tile(best.n_tiles, M, best.n_cta);
+    best.max_seg = max_segments_per_tile(best.n_tiles, M, best.vbins, best.n_cta);
     best.gmax = best.max_seg >= kFinishTwoLevelFrom ? (best.max_seg + kFinishGroup - 1) / kFinishGroup : 1;
     return best;
 }
@@ -461,6 +469,7 @@ int gw_ctx_create(gw_ctx **out, int64_t n_bins, const double *freqs_hz, int n_de
         ok = ok && (e = cudaStreamCreateWithFlags(&ctx->capture_stream, cudaStreamNonBlocking)) == cudaSuccess;
         if (!ok) { rc = cuda_fail(ctx, e); break; }
         ctx->host_graph = 1;
+        ctx->boundary_bins = kBoundaryBins;
     } while (0);
     cudaFree(dfreq); cudaFree(ddata); cudaFree(dpsd); cudaFree(di7);
     if (rc != GW_OK) {
@@ -561,23 +570,41 @@ int gw_ctx_host_graph(gw_ctx *ctx, int enable)
     return GW_OK;
 }
 
-int gw_plan_cta_segments(int64_t n_tiles, int64_t n_bins, int64_t n_ctas, int64_t cta, int max_rows, int64_t *rows6)
+int gw_plan_cta_segments(int64_t n_tiles, int64_t n_bins, int64_t boundary_bins, int64_t n_ctas, int64_t cta, int max_rows,
+                         int64_t *rows6)
 {
-    if (n_tiles < 1 || n_bins < 1 || n_ctas < 1 || cta < 0 || cta >= n_ctas || max_rows < 0 || (max_rows > 0 && !rows6))
+    if (n_tiles < 1 || n_bins < 1 || boundary_bins < 0 || n_ctas < 1 || cta < 0 || cta >= n_ctas || max_rows < 0 ||
+        (max_rows > 0 && !rows6))
         return GW_ERR_INVALID_ARG;
-    if ((double)n_tiles * (double)n_bins * (double)(n_ctas + 1) > 4.0e18) return GW_ERR_INVALID_ARG;
-    const int64_t work = n_tiles * n_bins;
+    if ((double)n_tiles * ((double)n_bins + (double)boundary_bins) * (double)(n_ctas + 1) > 4.0e18) return GW_ERR_INVALID_ARG;
+    const int64_t tile_len = n_bins + boundary_bins, work = flattened_work(n_tiles, n_bins, boundary_bins);
     const int64_t w_end = work_begin(cta + 1, work, n_ctas);
     int n = 0;
     for (int64_t w = work_begin(cta, work, n_ctas); w < w_end; ++n) {
-        const Segment s = segment_at(w, w_end, cta, n_bins, work, n_ctas);
+        const Segment s = segment_at(w, w_end, cta, n_bins, tile_len, work, n_ctas);
         if (n < max_rows) {
             int64_t *r = rows6 + 6 * n;
             r[0] = s.tile; r[1] = s.j0; r[2] = s.j1; r[3] = s.index; r[4] = s.count; r[5] = s.slot;
         }
-        w += s.j1 - s.j0;
+        w += s.len;
     }
     return n;
+}
+
+int gw_ctx_plan_boundary_bins(const gw_ctx *ctx, int64_t n_prop, int *boundary_bins)
+{
+    if (!ctx || n_prop < 1 || !boundary_bins) return GW_ERR_INVALID_ARG;
+    *boundary_bins = make_plan(ctx, n_prop).vbins;
+    return GW_OK;
+}
+
+int gw_ctx_boundary_bins(gw_ctx *ctx, int boundary_bins)
+{
+    if (!ctx || boundary_bins < 0 || boundary_bins > 4096) return GW_ERR_INVALID_ARG;
+    ctx->boundary_bins = boundary_bins;
+    for (int i = 0; i < 4; ++i) ctx->plan_n[i] = 0;
+    drop_host_graphs(ctx);
+    return GW_OK;
 }
 
 int gw_ctx_norms(const gw_ctx *ctx, double *i7_host)
@@ -628,7 +655,7 @@ static int lnl_batch_impl(gw_ctx *ctx, int64_t n_prop, const double *theta_dev, 
     if (p.gmax > 1 && (p.n_tiles * p.gmax * (int64_t)(2 * ctx->t.n_det) * p.props_per_cta > ctx->w.gpartial_doubles ||
                        p.n_tiles * p.gmax > ctx->w.n_gtickets))
         return GW_ERR_INVALID_ARG;
-    if ((double)p.n_tiles * (double)ctx->t.n_bins * (double)(p.n_cta + 1) > 4.0e18) return GW_ERR_INVALID_ARG;   // 64-bit range arithmetic
+    if ((double)p.n_tiles * (double)(ctx->t.n_bins + p.vbins) * (double)(p.n_cta + 1) > 4.0e18) return GW_ERR_INVALID_ARG;   // 64-bit range arithmetic
     if (ctx->timing) cudaEventRecord(ctx->ev[0], s);
     cudaError_t e = launch_setup(ctx->t, ctx->dets, ctx->gmst, ctx->spin_order, n_prop, theta_dev, ctx->w.rec,
                                  ctx->w.rec_stride, (double)p.lpp * ctx->t.delta_f, 1, theta_in_host_memory, s,

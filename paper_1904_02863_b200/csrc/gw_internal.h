@@ -92,6 +92,7 @@ struct Plan {
     int     gmax;         // groups per tile of the two-level finish: stride of the group workspace (>= 1)
     int     exclusive;    // 1: the grid has at most one CTA per SM and is launched so that no SM takes two
     int     cluster;      // > 0: aligned multi-lane grid whose n_chunks (= cluster) chunks per tile form a thread-block cluster
+    int     vbins;        // boundary bins between consecutive tiles in the flattened space (0 on aligned grids; see segment_at)
 };
 
 // ---- flattened work ranges (shared by the kernel, the planner and the CPU tests of the host logic) --------------
@@ -102,24 +103,41 @@ __host__ __device__ inline int64_t cta_of_position(int64_t p, int64_t work, int6
 {
     return ((p + 1) * n_cta + work - 1) / work - 1;
 }
+// size of the flattened space: n_tiles tiles of n_bins bins with vbins boundary positions between consecutive tiles
+__host__ __device__ inline int64_t flattened_work(int64_t n_tiles, int64_t n_bins, int64_t vbins)
+{
+    return n_tiles * (n_bins + vbins) - vbins;
+}
 // One segment = the part of a CTA's range that lies in one tile.
+// Boundary bins: a CTA whose range crosses a tile boundary pays a segment end (seed, partial store, fence, ticket) and a
+// second prologue, about as long as sweeping 30 bins.  So that such a CTA still finishes with the others, every tile but
+// the last is n_bins + vbins = tile_len positions long in the flattened space: the vbins positions behind a tile's last
+// bin hold no work, and a range that crosses them has that many bins less to sweep.  A range that only touches a tile's
+// boundary positions is a segment of no bins (j0 = j1 = n_bins): it contributes zeros and takes its ticket like any
+// other -- the hot kernel has no branch around a segment (a branch there costs the hot loop 5 % through ptxas's register
+// allocation).  vbins = 0 gives plain equal shares.
 struct Segment {
     int64_t tile, j0, j1;  // bins [j0, j1) of proposal tile `tile`
+    int64_t len;           // flattened positions of the range that lie in this tile (>= j1 - j0)
     int64_t first_cta;     // the CTA that holds the tile's first bin
     int     index;         // position among the tile's segments (ascending bins) = cta - first_cta
     int     count;         // segments of the tile
     int64_t slot;          // partial-sum slot = cta + tile: consecutive along a tile, unique over the grid
 };
-__host__ __device__ inline Segment segment_at(int64_t w, int64_t w_end, int64_t cta, int64_t n_bins, int64_t work,
-                                              int64_t n_cta)
+__host__ __device__ inline Segment segment_at(int64_t w, int64_t w_end, int64_t cta, int64_t n_bins, int64_t tile_len,
+                                              int64_t work, int64_t n_cta)
 {
     Segment s;
-    s.tile = w / n_bins;
-    s.j0 = w - s.tile * n_bins;
+    s.tile = w / tile_len;
+    const int64_t p0 = w - s.tile * tile_len;                 // position within the tile, boundary positions included
     const int64_t left = w_end - w;
-    s.j1 = (n_bins - s.j0 < left) ? n_bins : s.j0 + left;
-    s.first_cta = cta_of_position(s.tile * n_bins, work, n_cta);
-    const int64_t last_cta = cta_of_position(s.tile * n_bins + n_bins - 1, work, n_cta);
+    const int64_t p1 = (tile_len - p0 < left) ? tile_len : p0 + left;
+    s.len = p1 - p0;
+    s.j0 = p0 < n_bins ? p0 : n_bins;
+    s.j1 = p1 < n_bins ? p1 : n_bins;
+    s.first_cta = cta_of_position(s.tile * tile_len, work, n_cta);
+    const int64_t t_end = s.tile * tile_len + tile_len;       // one past the tile's last position (boundary positions included)
+    const int64_t last_cta = cta_of_position((t_end < work ? t_end : work) - 1, work, n_cta);
     s.index = (int)(cta - s.first_cta);
     s.count = (int)(last_cta - s.first_cta + 1);
     s.slot = cta + s.tile;

@@ -586,7 +586,8 @@ cudaError_t launch_waveform(const Tables &t, int64_t n_prop, const double *rec, 
 struct FusedArgs {
     const double *planes, *rec;
     int64_t n_pad, n_bins, n_prop, rec_stride;
-    int64_t work;            // n_tiles * n_bins: size of the flattened (tile, bin) space
+    int64_t tile_len;        // n_bins + boundary bins: positions per tile in the flattened space (gw_internal.h, segment_at)
+    int64_t work;            // flattened_work(n_tiles, n_bins, vbins): size of the flattened (tile, bin) space
     int64_t n_cta;           // CTAs of the grid: CTA k sweeps [k work / n_cta, (k+1) work / n_cta)
     int     lpp;
     int     gmax;            // groups per tile of the two-level finish (stride of gpartial / gtickets)
@@ -1104,9 +1105,9 @@ __global__ void __launch_bounds__(kThreads, NDET > 4 ? 1 : kMinCtas) fused_kerne
     uint32_t g = 0;
     bool first = true;
     for (int64_t w = work_begin(cta, a.work, a.n_cta); w < w_end;) {
-        const Segment seg = segment_at(w, w_end, cta, a.n_bins, a.work, a.n_cta);
+        const Segment seg = segment_at(w, w_end, cta, a.n_bins, a.tile_len, a.work, a.n_cta);
         fused_segment<NDET, MULTI, ISCO, TIDAL>(a, seg, g, first, smem_raw, s_ticket, s_relmax);
-        w += seg.j1 - seg.j0;
+        w += seg.len;
         first = false;
         if (w < w_end) __syncthreads();                      // s_ticket / s_relmax / stage buffers change hands
     }
@@ -1152,7 +1153,8 @@ cudaError_t launch_fused(const Tables &t, const Plan &plan, int64_t n_prop, cons
     FusedArgs a;
     a.planes = t.planes; a.rec = rec; a.n_pad = t.n_pad; a.n_bins = t.n_bins; a.n_prop = n_prop;
     a.rec_stride = rec_stride; a.lpp = plan.lpp; a.f0 = t.f0; a.delta_f = t.delta_f;
-    a.work = plan.n_tiles * t.n_bins; a.n_cta = plan.n_cta; a.gmax = plan.gmax; a.cluster = plan.cluster;
+    a.tile_len = t.n_bins + plan.vbins; a.work = flattened_work(plan.n_tiles, t.n_bins, plan.vbins);
+    a.n_cta = plan.n_cta; a.gmax = plan.gmax; a.cluster = plan.cluster;
     for (int i = 0; i < GW_MAX_DET; ++i) a.i7[i] = t.i7[i];
     a.partial = partial; a.tickets = tickets; a.lnl = lnl_out; a.parts = parts_out;
     a.gpartial = gpartial; a.gtickets = gtickets;
