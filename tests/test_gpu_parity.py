@@ -549,3 +549,42 @@ def test_host_variant_graph_path_matches_launch_by_launch(oracle, torch_cuda, ba
     assert np.array_equal(g_lnl, dev_lnl.cpu().numpy()) and np.array_equal(g_parts, dev_parts.cpu().numpy())
     assert np.array_equal(g_lnl, p_lnl) and np.array_equal(g_parts, p_parts) and np.array_equal(g_only, g_lnl)
     assert np.array_equal(g_rev, g_lnl[::-1]) and np.array_equal(p_rev, g_rev) and np.array_equal(pin_out, g_lnl)
+
+
+@pytest.mark.parametrize("lpp,n_ctas,vbins", [(1, 7, 0), (1, 7, 30), (1, 12, 30), (1, 10, 40), (4, 12, 10), (4, 6, 30),
+                                              (32, 4, 30), (32, 5, 20), (32, 61, 3), (2, 4, 30), (2, 148, 30)])
+@pytest.mark.parametrize("option", ["plain", "isco_cut", "tidal"])
+def test_balanced_grids_with_boundary_bins(oracle, torch_cuda, lpp, n_ctas, vbins, option):
+    """Pinned balanced grids (gw_ctx_force_grid: n_ctas CTAs share the flattened (tile, bin) space) with boundary bins
+    between the tiles (gw_ctx_boundary_bins), for one-lane and multi-lane layouts and the kernel variants: against the
+    oracle, run-to-run identical bits, and -- where the range arithmetic says so -- with CTAs whose range only touches a
+    tile's boundary positions (segments of no bins, which must contribute exact zeros)."""
+    torch = torch_cuda
+    from paper_1904_02863_b200 import GwContext, binding
+    cfg = inputs.CONFIGS["C1"].reduced(f_max=100.0, batch=2000 if lpp == 1 else 700)           # 321 bins
+    f, S, dets, d, th = make_problem(oracle, cfg)
+    kw, okw = {}, {}
+    if option == "isco_cut":
+        kw, okw = dict(isco_cut=1), dict(isco_cut=1)
+    if option == "tidal":
+        lam = inputs.tidal_lambdas(cfg, len(th))
+        th = np.ascontiguousarray(np.hstack([th, lam]))
+        kw, okw = dict(tidal_order=2), dict(lambdas=lam, tidal_order=2)
+    with GwContext(f, d, S, dets, cfg.gmst, spin_order=cfg.spin_order, max_batch=len(th), **kw) as ctx:
+        ctx.boundary_bins(vbins)
+        ctx.force_grid(lpp, n_ctas)
+        plan = ctx.plan(len(th))
+        used = ctx.plan_boundary_bins(len(th))
+        assert plan["lanes_per_prop"] == lpp and plan["n_ctas"] == n_ctas
+        thd = _dev(torch, th)
+        lnl, parts = ctx.lnl_batch(thd, want_parts=True)
+        lnl2, parts2 = ctx.lnl_batch(thd, want_parts=True)
+        torch.cuda.synchronize()
+        assert torch.equal(lnl, lnl2) and torch.equal(parts, parts2)
+    n_tiles = (len(th) + 256 // lpp - 1) // (256 // lpp)
+    rows = [binding.plan_cta_segments(n_tiles, f.size, n_ctas, k, boundary_bins=used) for k in range(n_ctas)]
+    n_empty = sum(int((r[:, 2] == r[:, 1]).sum()) for r in rows)
+    if (lpp, n_ctas, vbins) in ((1, 12, 30), (1, 10, 40), (4, 12, 10), (4, 6, 30), (32, 4, 30), (32, 5, 20), (2, 4, 30)):
+        assert used == vbins * lpp and n_empty > 0                        # these shapes do have zero-bin segments
+    ref = oracle.lnl(f, cfg.delta_f, d, S, dets, cfg.gmst, th[:, :11], cfg.spin_order, **okw)
+    assert_lnl_close(lnl.cpu().numpy(), parts.cpu().numpy(), ref[0], ref[1])
