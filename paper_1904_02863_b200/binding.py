@@ -54,14 +54,21 @@ def lib_path() -> str:
 
 
 _lib = None
+_lib_file = None
 
 
-def load_library():
-    """dlopen csrc/libgwlnl.so and declare the prototypes.  Fails loudly; never falls back."""
-    global _lib
+def load_library(variant_path: Optional[str] = None):
+    """dlopen csrc/libgwlnl.so and declare the prototypes.  Fails loudly; never falls back.
+
+    ``variant_path`` is for the diagnostic tools of this package only (timeline.py: the same sources built with
+    -DGW_TIMELINE): it must be given on the FIRST call of the process, before anything else has loaded the library; a
+    process uses one library throughout."""
+    global _lib, _lib_file
     if _lib is not None:
+        if variant_path is not None and os.path.abspath(variant_path) != _lib_file:
+            raise GwError(GW_ERR_INVALID_ARG, "load_library", f"{_lib_file} is already loaded in this process")
         return _lib
-    path = lib_path()
+    path = os.path.abspath(variant_path) if variant_path is not None else lib_path()
     if not os.path.exists(path):
         raise GwError(GW_ERR_CUDA, "load_library",
                       f"{path} is missing: build it with `python paper_1904_02863_b200/csrc/build.py` "
@@ -98,7 +105,7 @@ def load_library():
     for name in EXPORTS + TUNING_EXPORTS:
         if name not in ("gw_strerror", "gw_ctx_launch_count"):
             getattr(lib, name).restype = ci
-    _lib = lib
+    _lib, _lib_file = lib, path
     return lib
 
 

@@ -3,6 +3,9 @@
 
     csrc/libgwlnl.so    the product library: C-ABI of include/gwlnl.h, include/gwlnl_tuning.h, include/gwpop.h
     csrc/libgwprobe.so  measurement aids only (include/gwprobe.h): fp64-rate and HBM store / load bandwidth probes
+    csrc/libgwlnl_timeline.so  (on demand, build_timeline) the product sources compiled with -DGW_TIMELINE: the fused
+                        kernel's CTAs stamp a timeline (gw_kernels.cu); a diagnostic aid for timeline.py, never loaded by
+                        the product path
 
     python paper_1904_02863_b200/csrc/build.py [--force] [--verbose]
 
@@ -22,6 +25,7 @@ LIB = os.path.join(HERE, "libgwlnl.so")
 PROBE_SOURCES = ["gw_probe.cu"]
 PROBE_HEADERS = [os.path.join(INC, "gwprobe.h")]
 PROBE_LIB = os.path.join(HERE, "libgwprobe.so")
+TIMELINE_LIB = os.path.join(HERE, "libgwlnl_timeline.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
          "--fmad=false",            # every FMA in the kernels is explicit; no silent contraction elsewhere
@@ -57,6 +61,13 @@ def build_probe(force: bool = False) -> str:
         return PROBE_LIB
     subprocess.run([NVCC] + FLAGS + ["-o", PROBE_LIB] + PROBE_SOURCES, check=True, cwd=HERE)
     return PROBE_LIB
+
+
+def build_timeline(force: bool = False) -> str:
+    """The diagnostic variant of the product library with the per-CTA timeline stamps (timeline.py loads it)."""
+    if not force and _up_to_date(TIMELINE_LIB, SOURCES, HEADERS):
+        return TIMELINE_LIB
+    return build(force=True, defines=("GW_TIMELINE",), out=TIMELINE_LIB)
 
 
 if __name__ == "__main__":

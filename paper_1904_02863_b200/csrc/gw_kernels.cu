@@ -616,6 +616,34 @@ __device__ __forceinline__ double log_bessel_i0(double x)
 
 // The record fields the finish stage needs (CA_I and the cut index).  The cross-chunk finish loads them before the
 // ticket round trip so that their L2 latency is not added to the last CTA's serial chain.
+// ---- per-CTA timeline (diagnostic build only: -DGW_TIMELINE, csrc/build.py build_timeline, timeline.py) ----------------
+// Thread 0 of every CTA stores the nanosecond globaltimer (and, for the first eight stamps, clock64) into a caller-given
+// buffer of 32 words per CTA: 0 kernel entry, 1 sweep start / 2 sweep end / 3 ticket taken of the CTA's first segment,
+// 4 exit, 5-7 the same three for its last later segment, 8..23 stage starts of the first segment; 24..31 clock64 at
+// stamps 0..7.  Every stamp is stored at once, so no register is held across the sweep (ptxas: no spill, the hot loop
+// unchanged).  The product build compiles GW_STAMP to nothing.
+#ifdef GW_TIMELINE
+__device__ unsigned long long *g_timeline = nullptr;
+__device__ __forceinline__ unsigned long long timeline_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define GW_STAMP(k)                                                                                        \
+    do {                                                                                                   \
+        if (threadIdx.x == 0) {                                                                            \
+            unsigned long long *p_ = g_timeline;                                                           \
+            if (p_) {                                                                                      \
+                p_[(size_t)blockIdx.x * 32 + (k)] = timeline_ns();                                         \
+                if ((k) < 8) p_[(size_t)blockIdx.x * 32 + 24 + (k)] = (unsigned long long)clock64();       \
+            }                                                                                              \
+        }                                                                                                  \
+    } while (0)
+#else
+#define GW_STAMP(k) do { } while (0)
+#endif
+
 template <int NDET>
 struct FinishRec { double car[NDET], cai[NDET]; int64_t jcut; };
 
@@ -735,6 +763,7 @@ __device__ __forceinline__ void fused_segment(const FusedArgs &a, const Segment 
         n_issued = max(n_run, n_issued0);
     }
     int iters_total = 0;
+    GW_STAMP(first ? 1 : 5);
     for (int s = 0; s < n_stage; ++s) {
         const int buf = (int)((g + (uint32_t)s) % kStages);
         const uint32_t parity = ((g + (uint32_t)s) / kStages) & 1u;
@@ -745,6 +774,7 @@ __device__ __forceinline__ void fused_segment(const FusedArgs &a, const Segment 
             continue;
         }
         mbar_wait(&bars[buf], parity);
+        if (first) GW_STAMP(8 + (s < 15 ? s : 15));
         const double2 *P = sm + (size_t)buf * NP * kStageBins;
         const int iters = MULTI ? (cnt + lpp - 1) / lpp : cnt;
         // last kept bin of this proposal relative to the stage (isco_cut), in [-1, kStageBins]
@@ -896,6 +926,7 @@ __device__ __forceinline__ void fused_segment(const FusedArgs &a, const Segment 
         if (tid == 0 && s + kStages < n_run) issue_stage(s + kStages);   // n_run <= n_stage
     }
 
+    GW_STAMP(first ? 2 : 6);
     // seed (detectors >= 1): multiply by exp(+2 pi i f_last (tau_I - tau_0)), f_last = frequency of this
     // thread's last iteration
     {
@@ -1035,6 +1066,7 @@ __device__ __forceinline__ void fused_segment(const FusedArgs &a, const Segment 
         last_ticket = (unsigned)(n_groups - 1);
     }
     if (tid == 0) s_ticket = atomicAdd(&a.tickets[tile], 1u);
+    GW_STAMP(first ? 3 : 7);
     __syncthreads();
     if (s_ticket != last_ticket) return;
     // stage 2 (last CTA of the tile): segments (or group sums) added in index order
@@ -1094,6 +1126,7 @@ __global__ void __launch_bounds__(kThreads, NDET > 4 ? 1 : kMinCtas) fused_kerne
     __shared__ unsigned int s_ticket;
     __shared__ int s_relmax;
 
+    GW_STAMP(0);
     if (threadIdx.x == 0) {
         for (int s = 0; s < kStages; ++s) mbar_init(&bars[s], 1);
         mbar_fence_init();
@@ -1112,6 +1145,7 @@ __global__ void __launch_bounds__(kThreads, NDET > 4 ? 1 : kMinCtas) fused_kerne
         if (w < w_end) __syncthreads();                      // s_ticket / s_relmax / stage buffers change hands
     }
     if (first) pdl_wait_primary();                           // an empty range still orders itself after the setup kernel
+    GW_STAMP(4);
 }
 
 size_t fused_smem_bytes(int n_det)
@@ -1249,3 +1283,12 @@ int fused_ctas_per_sm(int n_det) { return (n_det >= 1 && n_det <= GW_MAX_DET) ? 
 int fused_cluster_ok(int n_det) { return (n_det >= 1 && n_det <= GW_MAX_DET) ? g_cluster_ok[n_det] : 0; }
 
 } // namespace gw
+
+#ifdef GW_TIMELINE
+// Diagnostic build only: the buffer (32 unsigned 64-bit words per CTA of the largest grid, device memory, zeroed by the
+// caller) the fused kernel's CTAs stamp into; NULL switches the stamps off.  Returns the cudaError_t.
+extern "C" int gw_timeline_set_buffer(unsigned long long *dev_ptr)
+{
+    return (int)cudaMemcpyToSymbol(gw::g_timeline, &dev_ptr, sizeof(dev_ptr));
+}
+#endif
