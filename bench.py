@@ -249,7 +249,7 @@ def run_population(args):
     step_ms = np.array([a.elapsed_time(b_) for a, b_ in zip(ev0, ev1)])
     value = B * args.steps / (step_ms.sum() * 1e-3)
     # kernel-level pass: every sample is the last of a burst of flushed steps without a host synchronisation in between,
-    # so that the SM clock is the loaded one (see run_ours and profiles/r2_clock_ramp.md)
+    # so that the SM clock is the loaded one (see run_ours and profiles/r2_timeline.md)
     step_est_ms = float(step_ms.mean()) + 0.05
     burst = int(min(64, max(4, np.ceil(3.0 / step_est_ms))))
     n_samples = int(max(10, min(args.steps, 2000.0 / (burst * step_est_ms))))
@@ -419,7 +419,7 @@ def run_ours(args):
     # ---- kernel-level pass (same stream, events inside the library around K3), flushed likewise ----
     # The library keeps one set of events per context, so a sample is read with a host synchronisation -- and an idle gap
     # of a few tens of microseconds is enough for the SM clock to fall by ~9 % (1.79 GHz against 1.95 GHz inside the fused
-    # kernel), while it needs ~2 ms of load to come back (profiles/r2_clock_ramp.md).  Every sample is therefore the LAST
+    # kernel), while it needs ~2 ms of load to come back (profiles/r2_timeline.md).  Every sample is therefore the LAST
     # call of a burst of flushed steps enqueued without a synchronisation, long enough (>= 3 ms) for the clock to be where
     # it is in the timed region above; kernel_ms_after_idle keeps the figure of a kernel that starts on an idle GPU.
     step_est_ms = total_ms / args.steps + 0.1                 # + the two flush kernels
@@ -479,7 +479,7 @@ def run_ours(args):
                 "kernel_ms_samples": n_samples, "kernel_ms_burst": burst,
                 "kernel_ms_note": "each sample: the last of `kernel_ms_burst` flushed steps enqueued without a host synchronisation "
                                   "(SM clock as in the timed region); kernel_ms_after_idle: one flushed step right after a host "
-                                  "synchronisation (the SM clock has fallen; profiles/r2_clock_ramp.md)",
+                                  "synchronisation (the SM clock has fallen; profiles/r2_timeline.md)",
                 "kernel_ms_after_idle": float(np.mean(k_idle_ms)),
                 "launch_floor_ms": floor_ms, "frac_net_of_launch_floor": flops_per_launch / ((fused_ms - floor_ms) * 1e-3) / 1e12 / peak,
                 "launch_floor_note": "kernel_ms is one launch between two CUDA events; an EMPTY kernel of the same launch shape timed "
