@@ -622,6 +622,10 @@ __device__ __forceinline__ double log_bessel_i0(double x)
 // 4 exit, 5-7 the same three for its last later segment, 8..23 stage starts of the first segment; 24..31 clock64 at
 // stamps 0..7.  Every stamp is stored at once, so no register is held across the sweep (ptxas: no spill, the hot loop
 // unchanged).  The product build compiles GW_STAMP to nothing.
+#ifndef GW_MULTI_UNROLL
+#define GW_MULTI_UNROLL 5
+#endif
+constexpr int kMultiUnroll = GW_MULTI_UNROLL;   // bins per unrolled trip of the lanes-interleaved sweep
 #ifdef GW_TIMELINE
 __device__ unsigned long long *g_timeline = nullptr;
 __device__ __forceinline__ unsigned long long timeline_ns()
@@ -890,7 +894,7 @@ __device__ __forceinline__ void fused_segment(const FusedArgs &a, const Segment 
             }
 #endif
         }
-#pragma unroll (MULTI ? 4 : 1)
+#pragma unroll (MULTI ? kMultiUnroll : 1)
         for (; it < iters; ++it) {
             int jj = MULTI ? sub + it * lpp : it;
             bool masked = false;
